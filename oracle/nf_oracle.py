@@ -1,0 +1,115 @@
+"""ctypes binding of ``nf_oracle.c`` (argument marshalling only; the arithmetic is in C).
+
+TEST INFRASTRUCTURE ONLY -- see the package docstring.  PAPER.md:337-349 (sec. 3.1) is
+the passage the C file follows.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nf_oracle.c")
+_LIB = os.path.join(_HERE, "libnf_oracle.so")
+_lib = None
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def build(force: bool = False) -> str:
+    """Compile ``nf_oracle.c`` with gcc -O2 (no fast-math) + OpenMP.  Returns the .so path."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        i64, f64, i32 = ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        vp = ctypes.c_void_p
+        lib.nfo_num_threads.restype = i32
+        lib.nfo_kernel.restype = f64
+        lib.nfo_kernel.argtypes = [f64, f64]
+        lib.nfo_bin.restype = i32
+        lib.nfo_bin.argtypes = [vp, i64, i32, f64, vp, vp, vp, vp]
+        lib.nfo_accel.restype = i32
+        lib.nfo_accel.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
+        lib.nfo_interactions.restype = i64
+        lib.nfo_interactions.argtypes = [vp, i32, i32]
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        name = {-1: "ARG", -2: "DOMAIN", -3: "NOMEM"}.get(rc, str(rc))
+        raise OracleError(f"{what} failed: NFO_ERR_{name}")
+
+
+def _pos32(pos) -> np.ndarray:
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    if pos.ndim != 2 or pos.shape[1] != 3:
+        raise ValueError("pos must be [n][3]")
+    return pos
+
+
+def num_threads() -> int:
+    return int(_load().nfo_num_threads())
+
+
+def kernel(r: float, eps: float) -> float:
+    """K(r): the acceleration on a sink from a unit-mass source at displacement d is d*K(|d|)."""
+    return float(_load().nfo_kernel(float(r), float(eps)))
+
+
+def bin_particles(pos, cpd: int, L: float):
+    """Returns dict(cid, count, offset, perm) as uint32 arrays."""
+    pos = _pos32(pos)
+    n = pos.shape[0]
+    C = cpd ** 3
+    cid = np.empty(n, np.uint32)
+    count = np.empty(C, np.uint32)
+    offset = np.empty(C + 1, np.uint32)
+    perm = np.empty(n, np.uint32)
+    rc = _load().nfo_bin(pos.ctypes.data, n, cpd, float(L), cid.ctypes.data, count.ctypes.data,
+                         offset.ctypes.data, perm.ctypes.data)
+    _check(rc, "nfo_bin")
+    return {"cid": cid, "count": count, "offset": offset, "perm": perm}
+
+
+def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=None) -> np.ndarray:
+    """float64 accelerations [m][3]; ``sinks`` = input indices to evaluate (default: all, input order)."""
+    pos = _pos32(pos)
+    n = pos.shape[0]
+    if binning is None:
+        binning = bin_particles(pos, cpd, L)
+    if sinks is None:
+        sp, m = None, n
+    else:
+        sinks = np.ascontiguousarray(sinks, dtype=np.int64)
+        sp, m = sinks.ctypes.data, sinks.shape[0]
+    acc = np.zeros((m, 3), np.float64)
+    rc = _load().nfo_accel(pos.ctypes.data, n, cpd, float(L), float(eps), int(R),
+                           binning["cid"].ctypes.data, binning["offset"].ctypes.data,
+                           binning["perm"].ctypes.data, sp, m, acc.ctypes.data)
+    _check(rc, "nfo_accel")
+    return acc
+
+
+def interactions(count, cpd: int, R: int = 2) -> int:
+    """Exact ordered-pair count of the definition (self pairs included)."""
+    count = np.ascontiguousarray(count, dtype=np.uint32)
+    v = int(_load().nfo_interactions(count.ctypes.data, cpd, R))
+    if v < 0:
+        raise OracleError("nfo_interactions: cpd < 2R+1")
+    return v

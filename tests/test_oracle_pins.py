@@ -1,0 +1,354 @@
+"""Pins of the float64 oracle to what the paper and the mathematics fix (CPU only).
+
+Every check here goes through something OTHER than the oracle's own formula: closed forms,
+invariants, special cases that reduce to a textbook all-pairs sum, brute force on tiny inputs
+by a different route (particle-wise minimum image + explicit cell mask), and the defining
+properties of the spline (C^2 contact with r^-3 at the spline radius, quadratic inside).
+Pin numbers P1..P15 follow SURVEY.md sec. 8(c).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ independent brute force
+def taylor_kernel(r, eps_s):
+    """K(r) built from the DEFINING PROPERTY, not the printed coefficients: r^-3 outside eps_s;
+    inside, the 2nd-order Taylor expansion of g(r) = r^-3 about r = eps_s."""
+    r = np.asarray(r, dtype=np.float64)
+    out = np.zeros_like(r)
+    nz = r > 0
+    if eps_s == 0.0:
+        out[nz] = r[nz] ** -3
+        return out
+    g, g1, g2 = eps_s ** -3, -3.0 * eps_s ** -4, 12.0 * eps_s ** -5
+    inside = nz & (r < eps_s)
+    outside = nz & ~inside
+    h = r[inside] - eps_s
+    out[inside] = g + g1 * h + 0.5 * g2 * h * h
+    out[outside] = r[outside] ** -3
+    return out
+
+
+def cells_of(pos, cpd, L):
+    c = np.floor(pos.astype(np.float64) * (cpd / L)).astype(np.int64)
+    return np.minimum(c, cpd - 1)
+
+
+def brute_min_image(pos, cpd, L, eps, R):
+    """All pairs, PARTICLE-wise minimum image, masked by wrapped cell offset max-norm <= R.
+    Equals the cell-image definition iff cpd >= 2R + 2 (P7)."""
+    x = pos.astype(np.float64)
+    c = cells_of(pos, cpd, L)
+    d = x[None, :, :] - x[:, None, :]              # d[i, j] = x_j - x_i
+    d -= L * np.round(d / L)
+    oc = c[None, :, :] - c[:, None, :]
+    oc = (oc + cpd // 2) % cpd - cpd // 2        # wrapped offset; |.| = cpd/2 ties are > R anyway
+    mask = (np.abs(oc).max(axis=2) <= R)
+    r = np.sqrt((d * d).sum(axis=2))
+    K = taylor_kernel(r, 2.16 * eps) * mask
+    return (d * K[:, :, None]).sum(axis=1)
+
+
+def brute_cell_image_allpairs(pos, cpd, L, eps):
+    """cpd == 2R+1: every cell is in every stencil exactly once, so the near field is an UNMASKED
+    all-pairs sum whose image is fixed by the wrapped cell offset (P8)."""
+    x = pos.astype(np.float64)
+    c = cells_of(pos, cpd, L)
+    R = (cpd - 1) // 2
+    oc = c[None, :, :] - c[:, None, :]
+    ow = (oc + R) % cpd - R                          # wrapped into [-R, R]
+    w = (ow - oc) // cpd                             # -1, 0, +1 box shifts
+    d = x[None, :, :] - x[:, None, :] + w * L
+    r = np.sqrt((d * d).sum(axis=2))
+    K = taylor_kernel(r, 2.16 * eps)
+    return (d * K[:, :, None]).sum(axis=1)
+
+
+def relerr(a, b):
+    return np.linalg.norm(a - b, axis=1) / np.maximum(np.linalg.norm(b, axis=1), 1e-300)
+
+
+# ------------------------------------------------------------------ kernel pins (P1-P6)
+def test_golden_two_body(oracle_mod):
+    """P1 + P10: closed-form two-particle cases (tests/golden/two_body.txt)."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "two_body.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) >= 12
+    for row in rows:
+        cpd, R, eps = int(row[0]), int(row[1]), float(row[2])
+        v = [float(t) for t in row[3:]]
+        pos = np.array([v[0:3], v[3:6]], dtype=np.float32)
+        assert np.array_equal(pos.astype(np.float64), np.array([v[0:3], v[3:6]]))  # dyadic: exact
+        a = oracle_mod.accel(pos, cpd, 1.0, eps, R)
+        exp = np.array(v[6:9])
+        assert np.allclose(a[0], exp, rtol=1e-14, atol=1e-12), (row, a[0])
+        assert np.allclose(a[1], -exp, rtol=1e-14, atol=1e-12), (row, a[1])   # antisymmetry
+
+
+def test_kernel_newtonian_outside(oracle_mod):
+    """P1/P6: beyond the spline radius the law is exactly r^-3 ('returns to exactly the 1/r^2
+    form'); eps = 0 is textbook Newton everywhere (P5)."""
+    eps = 0.01
+    for r in [0.0216, 0.0217, 0.05, 0.3, 1.7]:
+        assert oracle_mod.kernel(r, eps) == pytest.approx(r ** -3, rel=1e-15)
+    for r in [1e-9, 1e-4, 0.02, 3.0]:
+        assert oracle_mod.kernel(r, 0.0) == pytest.approx(r ** -3, rel=1e-15)
+    assert oracle_mod.kernel(0.0, eps) == 0.0 and oracle_mod.kernel(0.0, 0.0) == 0.0
+
+
+def test_kernel_spline_defining_properties(oracle_mod):
+    """P2: inside eps_s the kernel is a quadratic in r (third finite difference vanishes) with
+    value, first and second derivative equal to those of r^-3 at eps_s.  These four facts fix the
+    polynomial uniquely without quoting its coefficients."""
+    eps = 0.37
+    es = 2.16 * eps
+    K = lambda r: oracle_mod.kernel(r, eps)
+    # quadratic: third differences vanish anywhere inside
+    for r0 in [0.05 * es, 0.3 * es, 0.7 * es]:
+        h = 0.02 * es
+        d3 = K(r0 + 3 * h) - 3 * K(r0 + 2 * h) + 3 * K(r0 + h) - K(r0)
+        assert abs(d3) < 1e-12 * K(r0)
+    # one-sided derivatives at eps_s from inside (exact for a quadratic up to rounding)
+    h = 1e-3 * es
+    k0, k1, k2 = K(es - 1e-15), K(es - h), K(es - 2 * h)
+    first = (3 * k0 - 4 * k1 + k2) / (2 * h)
+    second = (k0 - 2 * k1 + k2) / (h * h)
+    assert k0 == pytest.approx(es ** -3, rel=1e-12)
+    assert first == pytest.approx(-3 * es ** -4, rel=1e-8)
+    assert second == pytest.approx(12 * es ** -5, rel=1e-6)
+    # and the independent Taylor construction agrees everywhere
+    rs = np.linspace(1e-6, 2 * es, 4001)
+    ref = taylor_kernel(rs, es)
+    got = np.array([K(r) for r in rs])
+    assert np.allclose(got, ref, rtol=1e-12)
+
+
+def test_kernel_plummer_equivalence(oracle_mod):
+    """P3: eps is 'Plummer-equivalent': the central force gradient K(0) matches the
+    Plummer law r/(r^2+eps^2)^1.5 -> r/eps^3 to within the 0.3% of 2.16 vs 10^(1/3)."""
+    eps = 0.013
+    k0 = oracle_mod.kernel(1e-12, eps)
+    assert k0 * eps ** 3 == pytest.approx(1.0, rel=0.01)
+    assert k0 * eps ** 3 == pytest.approx(10.0 / 2.16 ** 3, rel=1e-9)
+    # 'at a scale mildly larger than the softening length': eps < eps_s < 3 eps
+    r_newton = min(r for r in np.linspace(eps, 3 * eps, 2001)
+                   if oracle_mod.kernel(r, eps) == pytest.approx(r ** -3, rel=1e-14))
+    assert eps < r_newton <= 2.16 * eps * 1.001
+
+
+def test_force_maximum(oracle_mod):
+    """P4: F(r) = r K(r) peaks at u* = (30 - sqrt(180))/36 with F* = 2.01002/eps_s^2 (calculus on the
+    quadratic fixed by P2), and the softened force never exceeds the Newtonian one."""
+    eps = 0.2
+    es = 2.16 * eps
+    us = np.linspace(1e-4, 1.5, 150001)
+    F = np.array([u * es * oracle_mod.kernel(u * es, eps) for u in us])
+    i = F.argmax()
+    assert us[i] == pytest.approx((30 - math.sqrt(180)) / 36, abs=2e-5)
+    assert F[i] * es ** 2 == pytest.approx(2.01002, rel=1e-5)
+    assert np.all(F <= 1.0 / (us * es) ** 2 * (1 + 1e-12))
+
+
+def test_eps_irrelevant_when_all_pairs_far(oracle_mod):
+    """P6: if every separation exceeds eps_s the result is identical for eps and eps = 0."""
+    rng = np.random.default_rng(5)
+    # jittered 6^3 lattice, min separation > 0.1
+    g = (np.stack(np.meshgrid(*[np.arange(6)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / 6
+    pos = (g + rng.uniform(-0.02, 0.02, g.shape)).astype(np.float32)
+    a0 = oracle_mod.accel(pos, 6, 1.0, 0.0, 2)
+    a1 = oracle_mod.accel(pos, 6, 1.0, 0.03, 2)     # eps_s = 0.0648 < 0.12
+    assert np.array_equal(a0, a1)
+
+
+# ------------------------------------------------------------------ stencil / periodicity (P7-P10)
+@pytest.mark.parametrize("cpd,R,n,eps", [(6, 2, 400, 0.004), (7, 2, 500, 0.02), (4, 1, 200, 0.01),
+                                          (9, 2, 600, 0.0), (5, 0, 300, 0.01)])
+def test_brute_force_min_image(oracle_mod, cpd, R, n, eps):
+    """P7: independent route -- all pairs, particle minimum image, explicit cell-offset mask."""
+    rng = np.random.default_rng(100 + cpd)
+    pos = rng.random((n, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, cpd, 1.0, eps, R)
+    ref = brute_min_image(pos, cpd, 1.0, eps, R)
+    assert relerr(a, ref).max() < 1e-11
+
+
+@pytest.mark.parametrize("cpd", [5, 3, 1])
+def test_cpd_equals_stencil(oracle_mod, cpd):
+    """P8: cpd = 2R+1 -> unmasked all-pairs with the image fixed by the wrapped cell offset."""
+    R = (cpd - 1) // 2
+    rng = np.random.default_rng(7 + cpd)
+    pos = rng.random((350, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, cpd, 1.0, 0.01, R)
+    ref = brute_cell_image_allpairs(pos, cpd, 1.0, 0.01)
+    assert relerr(a, ref).max() < 1e-11
+
+
+def test_non_unit_box(oracle_mod):
+    """Same two routes with L != 1 (box shifts are multiples of L)."""
+    rng = np.random.default_rng(3)
+    L = 7.5
+    pos = (rng.random((400, 3)) * L).astype(np.float32)
+    pos[pos >= L] = 0
+    a = oracle_mod.accel(pos, 6, L, 0.03, 2)
+    assert relerr(a, brute_min_image(pos, 6, L, 0.03, 2)).max() < 1e-11
+
+
+def test_whole_cell_translation(oracle_mod):
+    """P9: on a dyadic grid a translation by one cell width (with wrap) leaves accelerations
+    unchanged and moves every particle to the neighbouring cell."""
+    rng = np.random.default_rng(11)
+    pos = (rng.integers(0, 1024, (700, 3)) / 1024.0).astype(np.float32)
+    a = oracle_mod.accel(pos, 8, 1.0, 0.004, 2)
+    shifted = ((pos.astype(np.float64) + np.array([0.125, 0.0, 0.875])) % 1.0).astype(np.float32)
+    b = oracle_mod.accel(shifted, 8, 1.0, 0.004, 2)
+    assert np.allclose(a, b, rtol=1e-12, atol=1e-9)
+    c0 = oracle_mod.bin_particles(pos, 8, 1.0)["cid"].astype(np.int64)
+    c1 = oracle_mod.bin_particles(shifted, 8, 1.0)["cid"].astype(np.int64)
+    cx, cy, cz = c0 // 64, (c0 // 8) % 8, c0 % 8
+    assert np.array_equal(c1, (((cx + 1) % 8) * 8 + cy) * 8 + (cz + 7) % 8)
+
+
+def test_stencil_reach(oracle_mod):
+    """P10: a source R cells away contributes, R+1 cells away does not -- for every axis, both
+    directions, through the periodic faces too."""
+    cpd, R = 8, 2
+    for axis in range(3):
+        for sgn in (+1, -1):
+            for base in (0, 3, 7):
+                sink = np.array([0.5 / cpd + 3.0 / cpd] * 3)
+                sink[axis] = (base + 0.5) / cpd
+                for k, expect in ((R, True), (R + 1, False)):
+                    src = sink.copy()
+                    src[axis] = ((base + sgn * k) % cpd + 0.5) / cpd
+                    pos = np.array([sink, src], dtype=np.float32)
+                    a = oracle_mod.accel(pos, cpd, 1.0, 1e-4, R)
+                    if expect:
+                        d = sgn * k / cpd
+                        assert a[0, axis] == pytest.approx(np.sign(d) / d ** 2, rel=1e-12)
+                    else:
+                        assert np.all(a == 0.0)
+
+
+# ------------------------------------------------------------------ whole-sum invariants (P11-P14)
+def test_total_force_vanishes(oracle_mod):
+    """P11: pair antisymmetry + symmetric stencil -> sum of all accelerations is 0."""
+    import nf_inputs
+    for idx, ns in [(1, 16), (4, 16)]:
+        cfg = nf_inputs.scaled(idx, ns, cpd=6)
+        pos = nf_inputs.generate(cfg).numpy()
+        a = oracle_mod.accel(pos, cfg.cpd, cfg.L, cfg.eps, 2)
+        assert np.abs(a.sum(axis=0)).max() < 1e-11 * np.abs(a).sum()
+
+
+def test_symmetric_lattice(oracle_mod):
+    """P12: one particle at every cell centre -> every acceleration is 0; with six satellites at
+    centre +- 2^-6 along each axis the centre particle still gets 0, the satellites get equal-
+    magnitude axis-aligned forces and every cell's force sum is 0."""
+    cpd = 8
+    g = (np.stack(np.meshgrid(*[np.arange(cpd)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / cpd
+    a = oracle_mod.accel(g.astype(np.float32), cpd, 1.0, 0.002, 2)
+    assert np.abs(a).max() < 1e-11
+    h = 2.0 ** -6
+    offs = np.array([[0, 0, 0], [h, 0, 0], [-h, 0, 0], [0, h, 0], [0, -h, 0], [0, 0, h], [0, 0, -h]])
+    pos = (g[:, None, :] + offs[None, :, :]).reshape(-1, 3).astype(np.float32)
+    a = oracle_mod.accel(pos, cpd, 1.0, 0.002, 2).reshape(-1, 7, 3)
+    scale = np.abs(a).max()
+    assert np.abs(a[:, 0]).max() < 1e-12 * scale
+    assert np.abs(a.sum(axis=1)).max() < 1e-12 * scale
+    mags = np.linalg.norm(a[:, 1:], axis=2)
+    assert np.allclose(mags, mags[0, 0], rtol=1e-12)
+    for k in range(1, 7):                       # axis-aligned
+        ax = (k - 1) // 2
+        other = [d for d in range(3) if d != ax]
+        assert np.abs(a[:, k][:, other]).max() < 1e-12 * scale
+
+
+def test_power_of_two_scaling(oracle_mod):
+    """P13: (pos, L, eps) * 2^k  ->  a * 2^-2k exactly (all float operations scale exactly)."""
+    rng = np.random.default_rng(21)
+    pos = rng.random((500, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, 6, 1.0, 0.01, 2)
+    b = oracle_mod.accel(pos * np.float32(8.0), 6, 8.0, 0.08, 2)
+    assert np.array_equal(a, b * 64.0)
+
+
+def test_shuffle_invariance(oracle_mod):
+    """P14: a permutation of the input order permutes the output and nothing else."""
+    rng = np.random.default_rng(33)
+    pos = rng.random((800, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, 7, 1.0, 0.01, 2)
+    p = rng.permutation(800)
+    b = oracle_mod.accel(pos[p], 7, 1.0, 0.01, 2)
+    assert np.allclose(b, a[p], rtol=1e-12, atol=1e-9)
+
+
+def test_sink_subset_matches_full(oracle_mod):
+    rng = np.random.default_rng(34)
+    pos = rng.random((600, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, 6, 1.0, 0.01, 2)
+    s = rng.choice(600, 50, replace=False)
+    b = oracle_mod.accel(pos, 6, 1.0, 0.01, 2, sinks=s)
+    assert np.array_equal(a[s], b)
+
+
+# ------------------------------------------------------------------ binning (P15)
+def check_binning(pos, cpd, L, b):
+    n = len(pos)
+    cid = cells_of(pos, cpd, L)
+    cid = (cid[:, 0] * cpd + cid[:, 1]) * cpd + cid[:, 2]
+    assert np.array_equal(b["cid"].astype(np.int64), cid)
+    assert np.array_equal(b["count"].astype(np.int64), np.bincount(cid, minlength=cpd ** 3))
+    assert b["offset"][0] == 0 and b["offset"][-1] == n
+    assert np.array_equal(np.diff(b["offset"].astype(np.int64)), b["count"].astype(np.int64))
+    assert np.array_equal(b["perm"].astype(np.int64), np.argsort(cid, kind="stable"))
+
+
+def test_binning_definition(oracle_mod):
+    rng = np.random.default_rng(41)
+    pos = rng.random((5000, 3), dtype=np.float32)
+    check_binning(pos, 9, 1.0, oracle_mod.bin_particles(pos, 9, 1.0))
+
+
+def test_binning_adversarial(oracle_mod):
+    cpd = 7
+    top = np.nextafter(np.float32(1.0), np.float32(0.0))
+    faces = np.array([[k / cpd, (k + 1) / cpd, 0.0] for k in range(cpd)], dtype=np.float64)
+    faces[faces >= 1.0] = top
+    cases = {
+        "one_cell": np.full((300, 3), 0.3, np.float32),
+        "faces": faces.astype(np.float32),
+        "top": np.full((5, 3), top, np.float32),
+        "zero": np.zeros((4, 3), np.float32),
+        "empty": np.zeros((0, 3), np.float32),
+    }
+    for name, pos in cases.items():
+        check_binning(pos, cpd, 1.0, oracle_mod.bin_particles(pos, cpd, 1.0))
+    b = oracle_mod.bin_particles(cases["top"], cpd, 1.0)
+    assert np.all(b["cid"] == cpd ** 3 - 1)
+
+
+def test_domain_errors(oracle_mod):
+    for bad in [1.0, -1e-9, np.nan, np.inf]:
+        pos = np.array([[0.5, 0.5, 0.5], [0.1, bad, 0.2]], dtype=np.float32)
+        with pytest.raises(oracle_mod.OracleError):
+            oracle_mod.bin_particles(pos, 5, 1.0)
+    with pytest.raises(oracle_mod.OracleError):
+        oracle_mod.accel(np.zeros((1, 3), np.float32), 4, 1.0, 0.01, 2)     # cpd < 2R+1 (C8)
+
+
+def test_interaction_count(oracle_mod):
+    rng = np.random.default_rng(51)
+    pos = rng.random((3000, 3), dtype=np.float32)
+    for cpd, R in [(6, 2), (5, 2), (7, 1)]:
+        b = oracle_mod.bin_particles(pos, cpd, 1.0)
+        c = b["count"].astype(np.int64).reshape(cpd, cpd, cpd)
+        box = np.zeros_like(c)
+        for ox in range(-R, R + 1):
+            for oy in range(-R, R + 1):
+                for oz in range(-R, R + 1):
+                    box += np.roll(c, (ox, oy, oz), axis=(0, 1, 2))
+        assert oracle_mod.interactions(b["count"], cpd, R) == int((c * box).sum())

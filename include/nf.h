@@ -1,0 +1,156 @@
+/*
+ * nf.h -- C-ABI boundary of the B200-native near-field direct gravity sum.
+ *
+ * The operation is the near-field half of the Abacus force split (arXiv:2110.11398; line numbers
+ * are /root/reference/PAPER.md):
+ *   - the periodic box of side L is a lattice of CPD^3 cubic cells, a slab is the CPD^2 cells at
+ *     fixed x                                                         (sec. 3.1)
+ *   - the near field of a particle is "the force arising from nearby cells", set by the near-field
+ *     radius R; every pair is in exactly one of near/far field and periodic images are kept
+ *
+ *   - it is "sourced by particles in neighboring cells out to radius R" and "computed by a direct,
+ *     O(N^2) summation with a compact spline softening kernel"        (R = 2: 347)
+ *   - the softening law "returns to exactly the 1/r^2 form at a scale mildly larger than the
+ *     softening length", lengths quoted Plummer-equivalent
+ *
+ * Every sink particle i receives   a_i = sum_j d_ij K(|d_ij|),   d_ij = x_j - x_i + w L,
+ * over all particles j of the (2R+1)^3 periodic cells around its own cell (w in {-1,0,+1}^3 is the
+ * box shift implied by the wrap of the CELL index), with G = 1, unit masses and
+ *   K(r) = r^-3                          for r >= eps_s  (or eps = 0),
+ *   K(r) = (10 - 15u + 6u^2)/eps_s^3     for u = r/eps_s < 1,      eps_s = 2.16 eps,
+ *   K(0) = 0 (self term and exactly coincident particles).
+ * PAPER.md does not print the spline; this is the documented reading (readings C2/C3).
+ *
+ * All pointers named *_dev are DEVICE pointers valid on the plan's CUDA device; *_host are HOST
+ * pointers (pinned memory makes the copies asynchronous).  The library never frees or keeps caller
+ * memory past the call unless stated.  No torch types cross this boundary.
+ *
+ * Return values: 0 = NF_OK, negative = error; nf_last_error() gives a thread-local message.
+ * There is NO CPU fallback: without a CUDA device every compute call fails with NF_ERR_CUDA.
+ */
+#ifndef NF_H
+#define NF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NF_OK            0
+#define NF_ERR_ARG      -1   /* null pointer, n < 0, n + 3 cpd^3 >= 2^32, cpd < 2R+1, cpd^3 >= 2^32, L <= 0, eps < 0, R < 0 or R > 4 */
+#define NF_ERR_DOMAIN   -2   /* a coordinate is non-finite or outside [0, L)  (reported by nf_bin) */
+#define NF_ERR_STATE    -3   /* nf_accel before a successful nf_bin */
+#define NF_ERR_NOMEM    -4   /* device allocation failed / caller workspace too small */
+#define NF_ERR_CUDA     -5   /* any CUDA runtime failure, including "no device" */
+
+typedef struct nf_plan nf_plan;     /* opaque; owns every internal device buffer */
+
+typedef struct nf_stats {
+    long long n;               /* particles last binned */
+    long long cells;           /* cpd^3 */
+    long long padded_slots;    /* slots of the cell-padded source arrays (>= n) */
+    long long units;           /* work units (sink chunks) of the last binning */
+    long long interactions;    /* exact ordered pair evaluations of the definition, self pairs included:
+                                  sum_c n_c * sum_{c' in stencil(c)} n_c'  */
+    float ms_bin;              /* device time of the last nf_bin   (CUDA events on the plan's stream) */
+    float ms_accel;            /* device time of the last nf_accel (direct-sum kernel incl. fused scatter) */
+    int   sm_count;            /* multiprocessors of the device */
+    int   clock_khz;           /* cudaDevAttrClockRate (max SM clock) */
+    int   accel_grid;          /* CTAs of the persistent direct-sum launch */
+    int   accel_block;         /* threads per CTA */
+    int   kernel_launches_bin; /* kernels launched by one nf_bin */
+    int   kernel_launches_accel; /* kernels launched by one nf_accel */
+} nf_stats;
+
+/*
+ * nf_plan_create -- the problem statement of PAPER.md:337-349.
+ *   cpd  cells per dimension (>= 2R+1 so that no cell appears twice in a stencil)
+ *   L    box side (> 0), positions live in [0, L)
+ *   eps  Plummer-equivalent softening length (>= 0; 0 = pure Newtonian)
+ *   R    near-field radius in cells (0..4; 2 in production)
+ * Host-only: validates, precomputes constants, allocates nothing of size O(n).
+ * Returns NULL on error (see nf_last_error()).
+ */
+nf_plan *nf_plan_create(int cpd, double L, double eps, int R);
+
+/*
+ * nf_bin -- steps S1-S5: cell ids, per-cell counts, exclusive offsets, STABLE counting sort
+ * (within a cell: ascending input index), cell-sorted source arrays, work-unit list.
+ *   pos_dev  [n][3] float32, input order, device memory, read only
+ *   n        0 <= n, n + 3 cpd^3 < 2^32.  n = 0 is a valid no-op.
+ * May be called repeatedly; each call invalidates the previous binning.  Enqueues on the plan's
+ * stream, then performs ONE 4-byte device-to-host read (the domain-error flag) and therefore
+ * synchronises that stream before returning.
+ * Errors: NF_ERR_ARG, NF_ERR_DOMAIN (no partial result promised), NF_ERR_NOMEM, NF_ERR_CUDA.
+ */
+int nf_bin(nf_plan *plan, const float *pos_dev, long long n);
+
+/*
+ * nf_accel -- steps S6-S7: the direct sum over the cell stencil and the scatter to input order.
+ *   acc_dev  [n][3] float32, device memory, OVERWRITTEN (not accumulated) with a_i for the
+ *            positions last binned, row i = input particle i.
+ * Asynchronous: returns after enqueueing on the plan's stream.
+ * Errors: NF_ERR_STATE (no successful nf_bin), NF_ERR_ARG, NF_ERR_CUDA.
+ */
+int nf_accel(nf_plan *plan, float *acc_dev);
+
+/* nf_destroy -- frees everything the plan allocated (never a caller workspace).  NULL-safe. */
+void nf_destroy(nf_plan *plan);
+
+/* ---- host-buffer entry points (end-to-end path: the copies are part of the call) ------------- */
+
+/* Copies pos_host [n][3] to a plan-owned device buffer (async if pinned) and runs nf_bin on it. */
+int nf_bin_host(nf_plan *plan, const float *pos_host, long long n);
+/* Runs nf_accel into a plan-owned device buffer and copies it to acc_host [n][3]; synchronises. */
+int nf_accel_host(nf_plan *plan, float *acc_host);
+
+/* ---- supporting exports (harness, tests; not part of the paper's problem statement) ---------- */
+
+const char *nf_last_error(void);
+
+/* CUDA stream (cudaStream_t as void*) all later calls enqueue on.  Default: the legacy stream 0. */
+int nf_set_stream(nf_plan *plan, void *cuda_stream);
+
+/* Bytes of workspace nf_bin needs for n particles on this plan. */
+size_t nf_workspace_bytes(const nf_plan *plan, long long n);
+/* Lend a device workspace (borrowed until nf_destroy or the next nf_set_workspace; 256-byte aligned).
+ * Without it the plan allocates (and grows) its own with cudaMalloc. */
+int nf_set_workspace(nf_plan *plan, void *dev_ptr, size_t bytes);
+
+/*
+ * Borrowed DEVICE pointers into the last binning (valid until the next nf_bin / nf_destroy):
+ *   cell_id [n]      cell of input particle i, id = (cx*cpd + cy)*cpd + cz (x slowest, z fastest)
+ *   count   [cpd^3]  particles per cell
+ *   offset  [cpd^3+1] exclusive prefix sum of count, offset[cpd^3] = n
+ *   perm    [n]      sorted slot s holds input particle perm[s]
+ * Any output pointer may be NULL.
+ */
+int nf_get_binning(const nf_plan *plan, const unsigned **cell_id, const unsigned **count,
+                   const unsigned **offset, const unsigned **perm);
+
+/*
+ * Borrowed DEVICE pointers to the internal source layout (for layout tests only):
+ *   poff [cpd^3+1]  first slot of each cell in the padded arrays (cells padded to multiples of 4)
+ *   x, y, z [padded_slots]  cell-corner-relative coordinates times *scale (a power of two);
+ *                   pad slots hold a far-away dummy.
+ */
+int nf_get_layout(const nf_plan *plan, const unsigned **poff, const float **x, const float **y,
+                  const float **z, double *scale);
+
+/* Fills *out; synchronises the plan's stream (event times and the interaction count live on the device). */
+int nf_get_stats(nf_plan *plan, nf_stats *out);
+
+/*
+ * Tuning knobs (integers).  Unknown key -> NF_ERR_ARG.
+ *   "variant"      0 = packed f32x2 pair kernel (default), 1 = scalar FP32 kernel
+ *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
+ *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
+ *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
+ */
+int nf_set_option(nf_plan *plan, const char *key, long long value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NF_H */

@@ -1,0 +1,275 @@
+"""Thin ctypes binding of ``include/nf.h`` -- argument marshalling only.
+
+Every step of the hot path (cell ids, histogram, prefix sums, stable sort, gather, scheduling,
+direct sum, scatter) runs in the CUDA kernels of ``libnf_b200.so``; torch is used for device
+memory, streams and nothing else.  The functions carry the C names (``nf_plan_create``,
+``nf_bin``, ``nf_accel``, ``nf_destroy``, ...); ``Plan`` is a convenience wrapper around them.
+
+There is no CPU fallback: if the library cannot be loaded, importing this module raises.
+Operation defined in PAPER.md:337-349 (sec. 3.1); see ``include/nf.h``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -1, -2, -3, -4, -5
+_ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
+
+EXPORTS = [
+    "nf_plan_create", "nf_bin", "nf_accel", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
+    "nf_get_layout", "nf_get_stats", "nf_set_option",
+]
+
+
+class NFError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_ERR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class nf_stats(ctypes.Structure):
+    _fields_ = [
+        ("n", ctypes.c_longlong), ("cells", ctypes.c_longlong), ("padded_slots", ctypes.c_longlong),
+        ("units", ctypes.c_longlong), ("interactions", ctypes.c_longlong),
+        ("ms_bin", ctypes.c_float), ("ms_accel", ctypes.c_float),
+        ("sm_count", ctypes.c_int), ("clock_khz", ctypes.c_int),
+        ("accel_grid", ctypes.c_int), ("accel_block", ctypes.c_int),
+        ("kernel_launches_bin", ctypes.c_int), ("kernel_launches_accel", ctypes.c_int),
+    ]
+
+
+def _load() -> ctypes.CDLL:
+    path = _build.LIB
+    if not os.path.exists(path) or _build.stale():
+        try:
+            _build.build()
+        except Exception as e:  # no nvcc on this box and no prebuilt library: fail loudly
+            if not os.path.exists(path):
+                raise ImportError(f"libnf_b200.so is missing and could not be built ({e}); "
+                                  "there is no CPU fallback") from e
+    lib = ctypes.CDLL(path)
+    vp, ll, i32, dbl = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double
+    pp = ctypes.POINTER(ctypes.c_void_p)
+    lib.nf_plan_create.restype = vp
+    lib.nf_plan_create.argtypes = [i32, dbl, dbl, i32]
+    lib.nf_bin.restype = i32
+    lib.nf_bin.argtypes = [vp, vp, ll]
+    lib.nf_accel.restype = i32
+    lib.nf_accel.argtypes = [vp, vp]
+    lib.nf_destroy.restype = None
+    lib.nf_destroy.argtypes = [vp]
+    lib.nf_bin_host.restype = i32
+    lib.nf_bin_host.argtypes = [vp, vp, ll]
+    lib.nf_accel_host.restype = i32
+    lib.nf_accel_host.argtypes = [vp, vp]
+    lib.nf_last_error.restype = ctypes.c_char_p
+    lib.nf_last_error.argtypes = []
+    lib.nf_set_stream.restype = i32
+    lib.nf_set_stream.argtypes = [vp, vp]
+    lib.nf_workspace_bytes.restype = ctypes.c_size_t
+    lib.nf_workspace_bytes.argtypes = [vp, ll]
+    lib.nf_set_workspace.restype = i32
+    lib.nf_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.nf_get_binning.restype = i32
+    lib.nf_get_binning.argtypes = [vp, pp, pp, pp, pp]
+    lib.nf_get_layout.restype = i32
+    lib.nf_get_layout.argtypes = [vp, pp, pp, pp, pp, ctypes.POINTER(dbl)]
+    lib.nf_get_stats.restype = i32
+    lib.nf_get_stats.argtypes = [vp, ctypes.POINTER(nf_stats)]
+    lib.nf_set_option.restype = i32
+    lib.nf_set_option.argtypes = [vp, ctypes.c_char_p, ll]
+    return lib
+
+
+_lib = _load()
+LIB_PATH = _build.LIB
+
+
+def nf_last_error() -> str:
+    return (_lib.nf_last_error() or b"").decode()
+
+
+def _check(rc: int):
+    if rc != NF_OK:
+        raise NFError(rc, nf_last_error())
+
+
+def _dev_f32(t: torch.Tensor, what: str) -> torch.Tensor:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+            and t.dim() == 2 and t.shape[1] == 3):
+        raise TypeError(f"{what} must be a contiguous CUDA float32 tensor of shape [n, 3]")
+    return t
+
+
+def _host_f32(t: torch.Tensor, what: str) -> torch.Tensor:
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+            and t.dim() == 2 and t.shape[1] == 3):
+        raise TypeError(f"{what} must be a contiguous CPU float32 tensor of shape [n, 3]")
+    return t
+
+
+# ---- the C calls, same names ------------------------------------------------------------------
+def nf_plan_create(cpd: int, L: float, eps: float, R: int = 2) -> int:
+    h = _lib.nf_plan_create(int(cpd), float(L), float(eps), int(R))
+    if not h:
+        raise NFError(NF_ERR_ARG, nf_last_error())
+    return h
+
+
+def nf_destroy(plan: int) -> None:
+    _lib.nf_destroy(plan)
+
+
+def nf_set_stream(plan: int, cuda_stream: int) -> None:
+    _check(_lib.nf_set_stream(plan, ctypes.c_void_p(cuda_stream)))
+
+
+def nf_bin(plan: int, pos: torch.Tensor) -> None:
+    pos = _dev_f32(pos, "pos")
+    _check(_lib.nf_bin(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0]))
+
+
+def nf_accel(plan: int, acc: torch.Tensor) -> None:
+    acc = _dev_f32(acc, "acc")
+    _check(_lib.nf_accel(plan, ctypes.c_void_p(acc.data_ptr())))
+
+
+def nf_bin_host(plan: int, pos_host: torch.Tensor) -> None:
+    pos_host = _host_f32(pos_host, "pos_host")
+    _check(_lib.nf_bin_host(plan, ctypes.c_void_p(pos_host.data_ptr()), pos_host.shape[0]))
+
+
+def nf_accel_host(plan: int, acc_host: torch.Tensor) -> None:
+    acc_host = _host_f32(acc_host, "acc_host")
+    _check(_lib.nf_accel_host(plan, ctypes.c_void_p(acc_host.data_ptr())))
+
+
+def nf_workspace_bytes(plan: int, n: int) -> int:
+    return int(_lib.nf_workspace_bytes(plan, int(n)))
+
+
+def nf_set_workspace(plan: int, ws: torch.Tensor | None) -> None:
+    if ws is None:
+        _check(_lib.nf_set_workspace(plan, None, 0))
+    else:
+        _check(_lib.nf_set_workspace(plan, ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()))
+
+
+def nf_set_option(plan: int, key: str, value: int) -> None:
+    _check(_lib.nf_set_option(plan, key.encode(), int(value)))
+
+
+def nf_get_stats(plan: int) -> dict:
+    st = nf_stats()
+    _check(_lib.nf_get_stats(plan, ctypes.byref(st)))
+    return {name: getattr(st, name) for name, _ in nf_stats._fields_}
+
+
+class _DevView:
+    """Borrowed device memory exposed through __cuda_array_interface__ (copied out by the caller)."""
+
+    def __init__(self, ptr: int, n: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, True), "version": 2}
+
+
+def _copy_out(ptr, n: int, typestr: str, dtype) -> torch.Tensor:
+    if n == 0 or not ptr:
+        return torch.empty(0, dtype=dtype, device="cuda")
+    return torch.as_tensor(_DevView(ptr, n, typestr), device="cuda").clone()
+
+
+def nf_get_binning(plan: int, n: int, ncells: int) -> dict:
+    """Copies of cell_id [n], count [C], offset [C+1], perm [n] as int32-typed CUDA tensors holding the
+    uint32 bit patterns (view them as uint32 on the host)."""
+    p = [ctypes.c_void_p() for _ in range(4)]
+    _check(_lib.nf_get_binning(plan, *[ctypes.byref(q) for q in p]))
+    torch.cuda.current_stream().synchronize()
+    sizes = [n, ncells, ncells + 1, n]
+    names = ["cid", "count", "offset", "perm"]
+    return {k: _copy_out(q.value, s, "<i4", torch.int32) for k, q, s in zip(names, p, sizes)}
+
+
+def nf_get_layout(plan: int, ncells: int) -> dict:
+    p = [ctypes.c_void_p() for _ in range(4)]
+    sc = ctypes.c_double()
+    _check(_lib.nf_get_layout(plan, *[ctypes.byref(q) for q in p], ctypes.byref(sc)))
+    poff = _copy_out(p[0].value, ncells + 1, "<i4", torch.int32)
+    total = int(poff[-1].item()) & 0xFFFFFFFF
+    out = {"poff": poff, "scale": sc.value}
+    for k, q in zip("xyz", p[1:]):
+        out[k] = _copy_out(q.value, total, "<f4", torch.float32)
+    return out
+
+
+# ---- convenience wrapper ----------------------------------------------------------------------
+class Plan:
+    """``with Plan(cpd, L, eps, R) as p: p.bin(pos); acc = p.accel()``"""
+
+    def __init__(self, cpd: int, L: float, eps: float, R: int = 2):
+        self.cpd, self.L, self.eps, self.R = int(cpd), float(L), float(eps), int(R)
+        self.ncells = self.cpd ** 3
+        self.n = 0
+        self._h = nf_plan_create(cpd, L, eps, R)
+
+    def close(self):
+        if self._h:
+            nf_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _use_current_stream(self):
+        nf_set_stream(self._h, torch.cuda.current_stream().cuda_stream)
+
+    def set_option(self, key: str, value: int):
+        nf_set_option(self._h, key, value)
+
+    def bin(self, pos: torch.Tensor):
+        self._use_current_stream()
+        nf_bin(self._h, pos)
+        self.n = pos.shape[0]
+
+    def accel(self, out: torch.Tensor | None = None) -> torch.Tensor:
+        self._use_current_stream()
+        if out is None:
+            out = torch.empty((self.n, 3), dtype=torch.float32, device="cuda")
+        nf_accel(self._h, out)
+        return out
+
+    def bin_host(self, pos_host: torch.Tensor):
+        self._use_current_stream()
+        nf_bin_host(self._h, pos_host)
+        self.n = pos_host.shape[0]
+
+    def accel_host(self, out_host: torch.Tensor) -> torch.Tensor:
+        self._use_current_stream()
+        nf_accel_host(self._h, out_host)
+        return out_host
+
+    def binning(self) -> dict:
+        return nf_get_binning(self._h, self.n, self.ncells)
+
+    def layout(self) -> dict:
+        return nf_get_layout(self._h, self.ncells)
+
+    def stats(self) -> dict:
+        return nf_get_stats(self._h)
+
+    def workspace_bytes(self, n: int) -> int:
+        return nf_workspace_bytes(self._h, n)
+
+    def set_workspace(self, ws: torch.Tensor | None):
+        self._ws = ws
+        nf_set_workspace(self._h, ws)

@@ -1,0 +1,323 @@
+// nf_api.cu -- the C-ABI of include/nf.h: plan life cycle, workspace, streams, introspection.
+// Host logic only; the kernels live in nf_bin.cu (S1-S5) and nf_direct.cu (S6-S7).
+#include "nf_internal.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace nf {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Carve the arena.  Called with base == NULL to get the size only.
+size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells)
+{
+    size_t off = 0;
+    char *b = (char *)base;
+    auto take = [&](size_t bytes) -> void * {
+        void *p = b ? (void *)(b + off) : nullptr;
+        off = align_up(off + bytes, 256);
+        return p;
+    };
+    const size_t N = (size_t)(n > 0 ? n : 0);
+    const size_t C = ncells;
+    const size_t nonempty = N < C ? N : C;
+    const size_t pmax = N + 3 * nonempty + 8;
+    const size_t umax = nonempty + N / kChunk + 2;
+    const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
+    const size_t sort_blocks = (nsort + kSortTile - 1) / kSortTile + 1;
+    const size_t scan_items = (256 * sort_blocks > C + 2 ? 256 * sort_blocks : C + 2);
+    ws.cid  = (uint32_t *)take(4 * (N + 1));
+    ws.keyA = (uint32_t *)take(4 * nsort);
+    ws.keyB = (uint32_t *)take(4 * nsort);
+    ws.valA = (uint32_t *)take(4 * nsort);
+    ws.valB = (uint32_t *)take(4 * nsort);
+    ws.radix_hist = (uint32_t *)take(4 * 256 * sort_blocks);
+    ws.count  = (uint32_t *)take(4 * (C + 1));
+    ws.offset = (uint32_t *)take(4 * (C + 2));
+    ws.poff   = (uint32_t *)take(4 * (C + 2));
+    ws.ubase  = (uint32_t *)take(4 * (C + 2));
+    ws.scan_tmp = (uint32_t *)take(4 * (scan_items / 2048 + 4096));
+    ws.x = (float *)take(4 * pmax);
+    ws.y = (float *)take(4 * pmax);
+    ws.z = (float *)take(4 * pmax);
+    ws.units        = (Unit *)take(sizeof(Unit) * umax);
+    ws.units_sorted = (Unit *)take(sizeof(Unit) * umax);
+    ws.bucket_hist  = (uint32_t *)take(4 * 256);
+    ws.interactions = (unsigned long long *)take(8 * 4);
+    ws.scalars      = (uint32_t *)take(4 * 64);
+    ws.bytes = off;
+    return off;
+}
+
+static int ensure_device(nf_plan *p)
+{
+    if (p->device >= 0) return NF_OK;
+    int dev = 0, cnt = 0;
+    cudaError_t e = cudaGetDeviceCount(&cnt);
+    if (e != cudaSuccess || cnt == 0) {
+        set_error("no CUDA device available (%s); this library has no CPU fallback",
+                  e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+        return NF_ERR_CUDA;
+    }
+    NF_CUDA_OK(cudaGetDevice(&dev));
+    NF_CUDA_OK(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    NF_CUDA_OK(cudaDeviceGetAttribute(&p->clock_khz, cudaDevAttrClockRate, dev));
+    for (int i = 0; i < 4; i++) NF_CUDA_OK(cudaEventCreate(&p->ev[i]));
+    p->device = dev;
+    return NF_OK;
+}
+
+static int ensure_workspace(nf_plan *p, long long n)
+{
+    Workspace tmp;
+    size_t need = carve(tmp, nullptr, n, p->k.ncells);
+    if (p->arena && p->arena_bytes >= need) {
+        if (p->ws_n != n) { carve(p->ws, p->arena, n, p->k.ncells); p->ws_n = n; }
+        return NF_OK;
+    }
+    if (p->arena && !p->arena_owned) {
+        set_error("caller workspace too small: have %zu bytes, need %zu", p->arena_bytes, need);
+        return NF_ERR_NOMEM;
+    }
+    if (p->arena) { cudaFree(p->arena); p->arena = nullptr; p->arena_bytes = 0; }
+    void *a = nullptr;
+    cudaError_t e = cudaMalloc(&a, need);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error("cudaMalloc of %zu workspace bytes failed: %s", need, cudaGetErrorString(e));
+        return NF_ERR_NOMEM;
+    }
+    p->arena = a; p->arena_bytes = need; p->arena_owned = true;
+    carve(p->ws, p->arena, n, p->k.ncells);
+    p->ws_n = n;
+    return NF_OK;
+}
+
+static int ensure_stage(nf_plan *p, long long n)
+{
+    size_t need = (size_t)(n > 0 ? n : 1) * 3 * sizeof(float);
+    if (p->stage_cap >= need) return NF_OK;
+    if (p->pos_stage) cudaFree(p->pos_stage);
+    if (p->acc_stage) cudaFree(p->acc_stage);
+    p->pos_stage = p->acc_stage = nullptr; p->stage_cap = 0;
+    if (cudaMalloc(&p->pos_stage, need) != cudaSuccess || cudaMalloc(&p->acc_stage, need) != cudaSuccess) {
+        cudaGetLastError();
+        set_error("cudaMalloc of host-path staging buffers (2 x %zu bytes) failed", need);
+        return NF_ERR_NOMEM;
+    }
+    p->stage_cap = need;
+    return NF_OK;
+}
+
+}  // namespace nf
+
+using namespace nf;
+
+extern "C" {
+
+const char *nf_last_error(void) { return g_err; }
+
+nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
+{
+    if (R < 0 || R > kMaxR) { set_error("R = %d outside [0, %d]", R, kMaxR); return nullptr; }
+    if (cpd < 2 * R + 1) { set_error("cpd = %d < 2R+1 = %d: a cell would appear twice in a stencil", cpd, 2 * R + 1); return nullptr; }
+    if ((double)cpd * cpd * cpd >= 4294967296.0) { set_error("cpd^3 >= 2^32"); return nullptr; }
+    if (!(L > 0.0) || !std::isfinite(L)) { set_error("L must be positive and finite"); return nullptr; }
+    if (!(eps >= 0.0) || !std::isfinite(eps)) { set_error("eps must be >= 0 and finite"); return nullptr; }
+    nf_plan *p = new (std::nothrow) nf_plan();
+    if (!p) { set_error("out of host memory"); return nullptr; }
+    memset(p, 0, sizeof(*p));
+    Consts &k = p->k;
+    k.cpd = cpd; k.R = R; k.ncells = (uint32_t)cpd * cpd * cpd;
+    k.L = L; k.cell_w = L / cpd; k.inv_cell_w = (double)cpd / L;
+    int e2 = 0;
+    (void)std::frexp(k.cell_w, &e2);              // cell_w = m 2^e2, m in [0.5, 1)
+    k.scale = std::ldexp(1.0, 1 - e2);            // cell_w * scale in [1, 2)
+    k.out_scale = k.scale * k.scale;
+    k.tiny = 1e-36f;
+    const double es = 2.16 * eps * k.scale;       // spline radius in scaled units
+    if (eps == 0.0) {
+        k.A = 3.0e38f; k.B = 0.f; k.C = 0.f;      // min(r^-3, 3e38): only r = 0 is capped, and 3e38 * 0 = 0
+    } else {
+        const double A = 10.0 / (es * es * es), B = -15.0 / (es * es * es * es), C = 6.0 / (es * es * es * es * es);
+        if (!(std::fabs(C) < 1e37) || !(std::fabs(B) < 1e37) || !(A < 1e37)) {
+            set_error("eps = %g is too small relative to the cell width %g for float32 spline coefficients; use eps = 0", eps, k.cell_w);
+            delete p;
+            return nullptr;
+        }
+        k.A = (float)A; k.B = (float)B; k.C = (float)C;
+    }
+    k.fast_ok = (2.16 * eps <= 0.999 * k.cell_w) ? 1 : 0;
+    p->eps = eps;
+    p->device = -1;
+    p->stream = 0;
+    p->ws_n = -1;
+    p->variant = 0; p->fastpath = 1; p->heavy_first = 1; p->ctas_per_sm = 0;
+    g_err[0] = 0;
+    return p;
+}
+
+void nf_destroy(nf_plan *p)
+{
+    if (!p) return;
+    if (p->arena && p->arena_owned) cudaFree(p->arena);
+    if (p->pos_stage) cudaFree(p->pos_stage);
+    if (p->acc_stage) cudaFree(p->acc_stage);
+    if (p->device >= 0) for (int i = 0; i < 4; i++) cudaEventDestroy(p->ev[i]);
+    delete p;
+}
+
+int nf_set_stream(nf_plan *p, void *s)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    p->stream = (cudaStream_t)s;
+    return NF_OK;
+}
+
+size_t nf_workspace_bytes(const nf_plan *p, long long n)
+{
+    if (!p || n < 0) return 0;
+    Workspace tmp;
+    return carve(tmp, nullptr, n, p->k.ncells);
+}
+
+int nf_set_workspace(nf_plan *p, void *dev_ptr, size_t bytes)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (dev_ptr && ((uintptr_t)dev_ptr & 255)) { set_error("workspace must be 256-byte aligned"); return NF_ERR_ARG; }
+    if (p->arena && p->arena_owned) cudaFree(p->arena);
+    p->arena = dev_ptr; p->arena_bytes = dev_ptr ? bytes : 0; p->arena_owned = false;
+    p->ws_n = -1; p->binned = false;
+    return NF_OK;
+}
+
+int nf_bin(nf_plan *p, const float *pos, long long n)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    p->binned = false;
+    if (n < 0) { set_error("n < 0"); return NF_ERR_ARG; }
+    if ((double)n + 3.0 * p->k.ncells + 16.0 >= 4294967296.0) { set_error("n + 3 cpd^3 >= 2^32"); return NF_ERR_ARG; }
+    if (!pos && n > 0) { set_error("null pos"); return NF_ERR_ARG; }
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    rc = ensure_workspace(p, n);
+    if (rc) return rc;
+    rc = launch_bin(p, pos, n);
+    if (rc) return rc;
+    p->n = n; p->binned = true;
+    return NF_OK;
+}
+
+int nf_accel(nf_plan *p, float *acc)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_accel called before a successful nf_bin"); return NF_ERR_STATE; }
+    if (!acc && p->n > 0) { set_error("null acc"); return NF_ERR_ARG; }
+    return launch_accel(p, acc);
+}
+
+int nf_bin_host(nf_plan *p, const float *pos_host, long long n)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    p->binned = false;
+    if (n < 0 || (!pos_host && n > 0)) { set_error("bad pos_host / n"); return NF_ERR_ARG; }
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    rc = ensure_stage(p, n);
+    if (rc) return rc;
+    if (n > 0) NF_CUDA_OK(cudaMemcpyAsync(p->pos_stage, pos_host, (size_t)n * 12, cudaMemcpyHostToDevice, p->stream));
+    return nf_bin(p, p->pos_stage, n);
+}
+
+int nf_accel_host(nf_plan *p, float *acc_host)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_accel_host called before a successful nf_bin"); return NF_ERR_STATE; }
+    if (!acc_host && p->n > 0) { set_error("null acc_host"); return NF_ERR_ARG; }
+    int rc = ensure_stage(p, p->n);
+    if (rc) return rc;
+    rc = launch_accel(p, p->acc_stage);
+    if (rc) return rc;
+    if (p->n > 0) NF_CUDA_OK(cudaMemcpyAsync(acc_host, p->acc_stage, (size_t)p->n * 12, cudaMemcpyDeviceToHost, p->stream));
+    NF_CUDA_OK(cudaStreamSynchronize(p->stream));
+    return NF_OK;
+}
+
+int nf_get_binning(const nf_plan *p, const unsigned **cell_id, const unsigned **count,
+                   const unsigned **offset, const unsigned **perm)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("no binning"); return NF_ERR_STATE; }
+    if (cell_id) *cell_id = p->ws.cid;
+    if (count) *count = p->ws.count;
+    if (offset) *offset = p->ws.offset;
+    if (perm) *perm = p->perm;
+    return NF_OK;
+}
+
+int nf_get_layout(const nf_plan *p, const unsigned **poff, const float **x, const float **y,
+                  const float **z, double *scale)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("no binning"); return NF_ERR_STATE; }
+    if (poff) *poff = p->ws.poff;
+    if (x) *x = p->ws.x;
+    if (y) *y = p->ws.y;
+    if (z) *z = p->ws.z;
+    if (scale) *scale = p->k.scale;
+    return NF_OK;
+}
+
+int nf_get_stats(nf_plan *p, nf_stats *out)
+{
+    if (!p || !out) { set_error("null argument"); return NF_ERR_ARG; }
+    memset(out, 0, sizeof(*out));
+    out->cells = p->k.ncells;
+    out->accel_block = kAccelThreads;
+    if (p->device < 0) return NF_OK;
+    out->sm_count = p->sm_count; out->clock_khz = p->clock_khz;
+    out->accel_grid = p->accel_grid;
+    out->kernel_launches_bin = p->launches_bin;
+    out->kernel_launches_accel = p->launches_accel;
+    NF_CUDA_OK(cudaStreamSynchronize(p->stream));
+    if (p->binned) {
+        out->n = p->n;
+        uint32_t sc[4] = {0, 0, 0, 0};
+        unsigned long long inter = 0;
+        if (p->n > 0) {
+            NF_CUDA_OK(cudaMemcpy(sc, p->ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost));
+            NF_CUDA_OK(cudaMemcpy(&inter, p->ws.interactions, 8, cudaMemcpyDeviceToHost));
+        }
+        out->units = sc[2]; out->padded_slots = sc[3]; out->interactions = (long long)inter;
+    }
+    if (p->have_bin_time) NF_CUDA_OK(cudaEventElapsedTime(&out->ms_bin, p->ev[0], p->ev[1]));
+    if (p->have_accel_time) NF_CUDA_OK(cudaEventElapsedTime(&out->ms_accel, p->ev[2], p->ev[3]));
+    return NF_OK;
+}
+
+int nf_set_option(nf_plan *p, const char *key, long long v)
+{
+    if (!p || !key) { set_error("null argument"); return NF_ERR_ARG; }
+    if (!strcmp(key, "variant") && (v == 0 || v == 1)) { p->variant = (int)v; return NF_OK; }
+    if (!strcmp(key, "fastpath") && (v == 0 || v == 1)) { p->fastpath = (int)v; return NF_OK; }
+    if (!strcmp(key, "heavy_first") && (v == 0 || v == 1)) { p->heavy_first = (int)v; p->binned = false; return NF_OK; }
+    if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
+    set_error("unknown option or bad value: %s = %lld", key, v);
+    return NF_ERR_ARG;
+}
+
+}  // extern "C"

@@ -1,0 +1,101 @@
+// nf_internal.h -- plan state and kernel launchers shared by the three translation units of
+// libnf_b200.so.  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/nf.h"
+
+namespace nf {
+
+// ---- compile-time shape of the direct-sum kernel -------------------------------------------
+constexpr int kMaxR          = 4;                 // (2R+1) <= 9 pieces per stage
+constexpr int kMaxPieces     = 2 * kMaxR + 1;
+constexpr int kConsumerWarps = 4;                 // sink lanes per CTA = 128
+constexpr int kChunk         = 32 * kConsumerWarps;   // sinks per work unit
+constexpr int kTile          = 512;               // source slots per pipeline stage (multiple of 4)
+constexpr int kStages        = 3;                 // TMA pipeline depth
+constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
+constexpr float kDummy       = 36028797018963968.0f;        // 2^55: pad-slot coordinate, contributes exactly 0
+
+// ---- radix sort shape ----------------------------------------------------------------------
+constexpr int kSortWarps   = 8;
+constexpr int kSortThreads = 32 * kSortWarps;
+constexpr int kSortItems   = 16;                          // keys per thread
+constexpr int kSortTile    = kSortThreads * kSortItems;   // 4096 keys per block
+
+struct Unit {            // one work unit: a chunk of <= kChunk sinks of one cell
+    uint32_t cell;
+    uint32_t k0;         // first sink within the cell
+    uint32_t nk;         // sinks in the chunk
+    uint32_t cost_hi;    // Sum of stencil counts (sources per sink), saturated
+};
+
+struct Workspace {       // carved out of one arena; all 256-byte aligned
+    uint32_t *cid, *keyA, *keyB, *valA, *valB;   // [n]
+    uint32_t *radix_hist;                         // [256 * sort_blocks]
+    uint32_t *count, *offset, *poff, *ubase;      // [C], [C+1], [C+1], [C+1]
+    uint32_t *scan_tmp;                           // block sums
+    float *x, *y, *z;                             // [P_max]
+    Unit *units, *units_sorted;                   // [U_max]
+    uint32_t *bucket_hist;                        // [64] + cursor
+    unsigned long long *interactions;             // [1]
+    uint32_t *scalars;                            // [16]: 0 error flag, 1 unit counter, 2 n_units, 3 padded total
+    size_t bytes;
+};
+
+struct Consts {          // everything the kernels need about the problem, by value
+    int cpd, R;
+    uint32_t ncells;
+    double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L
+    double scale;                   // power of two with cell_w*scale in [1,2)
+    float A, B, C;                  // spline in scaled units: t(r) = A + B r + C r^2
+    float tiny;
+    int fast_ok;                    // eps_s <= 0.999 cell_w: cells with max-norm offset >= 2 are pure Newtonian
+    double out_scale;               // scale^2
+};
+
+}  // namespace nf
+
+struct nf_plan {
+    nf::Consts k;
+    double eps;
+    int device;
+    int sm_count, clock_khz;
+    cudaStream_t stream;
+    // workspace
+    void *arena;  size_t arena_bytes;  bool arena_owned;
+    nf::Workspace ws;
+    long long ws_n;                 // n the carve-up was made for (-1 = none)
+    // state of the last binning
+    long long n;  bool binned;
+    long long n_units;
+    int sort_passes;
+    const uint32_t *perm, *sorted_keys;
+    // host-buffer path
+    float *pos_stage; float *acc_stage; size_t stage_cap;   // device staging for *_host calls
+    // options
+    int variant, fastpath, heavy_first, ctas_per_sm;
+    // stats
+    cudaEvent_t ev[4];
+    bool have_bin_time, have_accel_time;
+    int accel_grid, launches_bin, launches_accel;
+};
+
+namespace nf {
+void set_error(const char *fmt, ...);
+size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells);   // base may be NULL (size only)
+int  launch_bin(nf_plan *p, const float *pos, long long n);             // S1-S5 (nf_bin.cu)
+int  launch_accel(nf_plan *p, float *acc);                               // S6-S7 (nf_direct.cu)
+int  accel_max_ctas_per_sm(int variant);
+}
+#define NF_CUDA_OK(call)                                                                        \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            nf::set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return NF_ERR_CUDA;                                                                 \
+        }                                                                                       \
+    } while (0)

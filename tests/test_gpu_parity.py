@@ -1,0 +1,245 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C-ABI binding, against the
+float64 oracle on the same seeded float32 inputs.  Binning and permutation bit-exact; accelerations
+within BASELINE.json's tolerance (99.9 % of particles <= 1e-5, max <= 1e-3)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import nf_inputs
+from nf_testlib import (assert_binning_equal, assert_parity, gpu_run, rel_errors, sample_sinks, u32)
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def full_check(oracle_mod, pos_cpu, cpd, L, eps, R=2, options=None, what=""):
+    out = gpu_run(pos_cpu, cpd, L, eps, R, options, want_binning=True)
+    pos = pos_cpu.numpy()
+    b = oracle_mod.bin_particles(pos, cpd, L)
+    assert_binning_equal(out["binning"], b)
+    ref = oracle_mod.accel(pos, cpd, L, eps, R, binning=b)
+    st = assert_parity(out["acc"], ref, what)
+    assert out["stats"]["interactions"] == oracle_mod.interactions(b["count"], cpd, R)
+    return st, out
+
+
+# ---------------------------------------------------------------- the five configs, small and full
+def test_config1_full(oracle_mod):
+    cfg = nf_inputs.config(1)
+    st, out = full_check(oracle_mod, nf_inputs.generate(cfg), cfg.cpd, cfg.L, cfg.eps, cfg.R, what=cfg.name)
+    print(cfg.name, st, out["stats"])
+
+
+def test_config1_shuffled(oracle_mod):
+    cfg = nf_inputs.config(1)
+    pos = nf_inputs.generate(cfg)
+    perm = torch.randperm(pos.shape[0], generator=torch.Generator().manual_seed(7))
+    full_check(oracle_mod, pos[perm].contiguous(), cfg.cpd, cfg.L, cfg.eps, cfg.R, what="config1 shuffled")
+
+
+@pytest.mark.parametrize("idx,n_side,cpd", [(2, 48, 12), (3, 40, 10), (4, 40, 10), (5, 40, 10)])
+def test_scaled_configs_full(oracle_mod, idx, n_side, cpd):
+    """Same recipes at sizes the oracle finishes in seconds; several tiles, ragged tails, heavy cells."""
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    st, out = full_check(oracle_mod, nf_inputs.generate(cfg), cfg.cpd, cfg.L, cfg.eps, cfg.R, what=cfg.name)
+    print(cfg.name, st)
+
+
+@pytest.mark.parametrize("variant,fastpath", [(1, 1), (0, 0), (1, 0)])
+def test_kernel_variants(oracle_mod, variant, fastpath):
+    cfg = nf_inputs.scaled(4, 32, 8)
+    full_check(oracle_mod, nf_inputs.generate(cfg), cfg.cpd, cfg.L, cfg.eps, cfg.R,
+               options={"variant": variant, "fastpath": fastpath}, what=f"variant{variant} fast{fastpath}")
+
+
+def sampled_check(oracle_mod, cfg, device="cpu"):
+    pos_dev = nf_inputs.generate(cfg, device=device)
+    pos_cpu = pos_dev.cpu()
+    pos = pos_cpu.numpy()
+    out = gpu_run(pos_cpu, cfg.cpd, cfg.L, cfg.eps, cfg.R, want_binning=True)
+    b = oracle_mod.bin_particles(pos, cfg.cpd, cfg.L)
+    assert_binning_equal(out["binning"], b)
+    assert out["stats"]["interactions"] == oracle_mod.interactions(b["count"], cfg.cpd, cfg.R)
+    rng = np.random.default_rng(cfg.seed)
+    sinks = sample_sinks(b["count"], b["offset"], b["perm"], cfg.cpd, rng)
+    ref = oracle_mod.accel(pos, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=sinks, binning=b)
+    st = assert_parity(out["acc"][sinks], ref, cfg.name + " (sampled)")
+    # property that holds at any size: total force vanishes (pair antisymmetry), within FP32 bounds
+    a = out["acc"]
+    assert np.abs(a.sum(axis=0)).max() <= 2e-6 * np.abs(a).sum()
+    print(cfg.name, "sampled sinks", len(sinks), st, out["stats"])
+
+
+def test_config2_full_size_sampled(oracle_mod):
+    sampled_check(oracle_mod, nf_inputs.config(2))
+
+
+def test_config3_full_size_sampled(oracle_mod):
+    sampled_check(oracle_mod, nf_inputs.config(3))
+
+
+def test_config4_full_size_sampled(oracle_mod):
+    sampled_check(oracle_mod, nf_inputs.config(4), device="cuda")
+
+
+# ---------------------------------------------------------------- closed forms through the GPU
+def test_golden_two_body_gpu():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "two_body.txt")) if l.strip() and l[0] != "#"]
+    for row in rows:
+        cpd, R, eps = int(row[0]), int(row[1]), float(row[2])
+        v = [float(t) for t in row[3:]]
+        pos = torch.tensor([v[0:3], v[3:6]], dtype=torch.float32)
+        a = gpu_run(pos, cpd, 1.0, eps, R)["acc"]
+        exp = np.array(v[6:9])
+        scale = max(np.abs(exp).max(), 1e-30)
+        assert np.abs(a[0] - exp).max() <= 2e-6 * scale, (row, a)
+        assert np.abs(a[1] + exp).max() <= 2e-6 * scale, (row, a)
+        if not exp.any():
+            assert not a.any()                       # exact zeros stay exact
+
+
+def test_symmetric_lattice_gpu():
+    """Reading C13: where the exact answer is 0, |a_gpu| <= 1e-5 * sum of pair-force magnitudes."""
+    cpd = 8
+    g = (np.stack(np.meshgrid(*[np.arange(cpd)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / cpd
+    a = gpu_run(torch.tensor(g, dtype=torch.float32), cpd, 1.0, 0.002, 2)["acc"]
+    pair_sum = 124 * 64.0            # loose upper bound: 124 neighbours at >= 1/8
+    assert np.abs(a).max() <= 1e-5 * pair_sum
+
+
+# ---------------------------------------------------------------- degenerate and edge cases
+def test_empty_and_single():
+    import paper_2110_11398_b200 as nf
+    with nf.Plan(7, 1.0, 0.01, 2) as p:
+        p.bin(torch.zeros((0, 3), device="cuda"))
+        assert p.accel().shape == (0, 3)
+        p.bin(torch.tensor([[0.3, 0.9, 0.1]], device="cuda"))
+        a = p.accel()
+        torch.cuda.synchronize()
+        assert a.shape == (1, 3) and not a.cpu().numpy().any()
+        assert p.stats()["interactions"] == 1
+
+
+def test_one_heavy_cell(oracle_mod):
+    """All particles in one cell: many sink chunks, sources tiled through several pipeline stages."""
+    g = torch.Generator().manual_seed(3)
+    pos = (torch.rand((3001, 3), generator=g) * (1.0 / 6) * 0.999 + 2.0 / 6).to(torch.float32)
+    full_check(oracle_mod, pos, 6, 1.0, 2e-3, 2, what="one heavy cell")
+
+
+def test_coincident_particles(oracle_mod):
+    g = torch.Generator().manual_seed(4)
+    pos = torch.rand((500, 3), generator=g)
+    pos = torch.cat([pos, pos[:100]]).contiguous()           # 100 exact duplicates
+    full_check(oracle_mod, pos, 5, 1.0, 0.01, 2, what="coincident")
+    full_check(oracle_mod, pos, 5, 1.0, 0.0, 2, what="coincident eps=0")
+
+
+@pytest.mark.parametrize("cpd,R,eps,L", [(5, 2, 0.01, 1.0), (3, 1, 0.02, 1.0), (1, 0, 0.01, 1.0), (7, 3, 0.005, 1.0),
+                                         (9, 4, 0.004, 1.0), (6, 0, 0.01, 1.0), (6, 2, 0.2, 1.0), (6, 2, 0.0, 1.0),
+                                         (8, 2, 0.03, 7.5), (8, 2, 25.0, 2000.0), (16, 2, 1e-5, 2.0 ** -10)])
+def test_parameter_sweep(oracle_mod, cpd, R, eps, L):
+    """cpd = 2R+1 (every cell in every stencil), R = 0..4, eps = 0, eps_s larger than a cell (no fast
+    path), non-unit and non-dyadic box sizes."""
+    g = torch.Generator().manual_seed(cpd * 10 + R)
+    pos = (torch.rand((4000, 3), generator=g, dtype=torch.float64) * L).to(torch.float32)
+    pos[pos >= L] = 0.0
+    full_check(oracle_mod, pos.contiguous(), cpd, L, eps, R, what=f"cpd{cpd} R{R} eps{eps} L{L}")
+
+
+def test_adversarial_binning(oracle_mod):
+    cpd = 7
+    top = np.nextafter(np.float32(1.0), np.float32(0.0))
+    faces = np.array([[k / cpd, (k + 1) / cpd, 0.0] for k in range(cpd)], dtype=np.float64)
+    faces[faces >= 1.0] = top
+    rng = np.random.default_rng(0)
+    cases = {
+        "faces": faces.astype(np.float32),
+        "top": np.full((5, 3), top, np.float32),
+        "zero": np.zeros((4, 3), np.float32),
+        "mixed": np.concatenate([faces.astype(np.float32), rng.random((5000, 3), dtype=np.float32),
+                                 np.full((300, 3), 0.3, np.float32)]),
+    }
+    for name, pos in cases.items():
+        out = gpu_run(torch.from_numpy(pos), cpd, 1.0, 0.01, 2, want_binning=True)
+        assert_binning_equal(out["binning"], oracle_mod.bin_particles(pos, cpd, 1.0))
+
+
+def test_layout_is_lossless():
+    """sorted cell-relative coordinates / scale + corner == input positions, exactly (host-side check of
+    the Sterbenz argument in DESIGN.md); pad slots hold the dummy."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.config(1)
+    pos = nf_inputs.generate(cfg)
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
+        p.bin(pos.cuda())
+        b = {k: u32(v) for k, v in p.binning().items()}
+        lay = p.layout()
+    poff = u32(lay["poff"]).astype(np.int64)
+    cnt = b["count"].astype(np.int64)
+    assert np.array_equal(np.diff(poff), (cnt + 3) // 4 * 4)
+    cid_sorted = np.repeat(np.arange(cfg.cpd ** 3), cnt)
+    slot = np.repeat(poff[:-1], cnt) + (np.arange(len(cid_sorted)) - np.repeat(b["offset"][:-1].astype(np.int64), cnt))
+    w = cfg.L / cfg.cpd
+    p64 = pos.numpy().astype(np.float64)[b["perm"]]
+    for d, (name, cidx) in enumerate(zip("xyz", [cid_sorted // cfg.cpd ** 2, (cid_sorted // cfg.cpd) % cfg.cpd, cid_sorted % cfg.cpd])):
+        corner = (cidx.astype(np.float64) * w).astype(np.float32).astype(np.float64)
+        rec = lay[name].cpu().numpy().astype(np.float64)[slot] / lay["scale"] + corner
+        assert np.array_equal(rec, p64[:, d])
+    real = np.zeros(poff[-1], bool)
+    real[slot] = True
+    assert np.all(lay["x"].cpu().numpy()[~real] == 2.0 ** 55)
+
+
+def test_rebin_workspace_stream(oracle_mod):
+    """nf_bin may be called repeatedly with new n; caller-lent workspace; non-default stream."""
+    import paper_2110_11398_b200 as nf
+    g = torch.Generator().manual_seed(9)
+    with nf.Plan(6, 1.0, 0.004, 2) as p:
+        ws = torch.empty(p.workspace_bytes(6000) + 256, dtype=torch.uint8, device="cuda")
+        p.set_workspace(ws)
+        s = torch.cuda.Stream()
+        for n in (6000, 100, 3000):
+            pos = torch.rand((n, 3), generator=g)
+            with torch.cuda.stream(s):
+                p.bin(pos.cuda())
+                a = p.accel()
+            s.synchronize()
+            ref = oracle_mod.accel(pos.numpy(), 6, 1.0, 0.004, 2)
+            assert_parity(a.cpu().numpy().astype(np.float64), ref, f"rebin n={n}")
+        with pytest.raises(nf.NFError) as e:
+            p.bin(torch.rand((100000, 3), device="cuda"))
+        assert e.value.code == nf.binding.NF_ERR_NOMEM
+
+
+def test_host_entry_points(oracle_mod):
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.scaled(1, 24, 6)
+    pos = nf_inputs.generate(cfg).pin_memory()
+    out = torch.empty_like(pos).pin_memory()
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
+        p.bin_host(pos)
+        p.accel_host(out)
+    ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
+    assert_parity(out.numpy().astype(np.float64), ref, "host entry points")
+
+
+def test_errors_gpu():
+    import paper_2110_11398_b200 as nf
+    B = nf.binding
+    with nf.Plan(5, 1.0, 0.01, 2) as p:
+        with pytest.raises(nf.NFError) as e:
+            p.accel(torch.empty((3, 3), device="cuda"))
+        assert e.value.code == B.NF_ERR_STATE
+        for bad in (1.0, -1e-9, float("nan"), float("inf")):
+            pos = torch.tensor([[0.5, 0.5, 0.5], [0.1, bad, 0.2]], device="cuda")
+            with pytest.raises(nf.NFError) as e:
+                p.bin(pos)
+            assert e.value.code == B.NF_ERR_DOMAIN
+            with pytest.raises(nf.NFError):
+                p.accel(torch.empty((2, 3), device="cuda"))
+        p.bin(torch.rand((10, 3), device="cuda"))      # the plan recovers
+        p.accel()

@@ -175,7 +175,7 @@ class _DevView:
     """Borrowed device memory exposed through __cuda_array_interface__ (copied out by the caller)."""
 
     def __init__(self, ptr: int, n: int, typestr: str):
-        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, True), "version": 2}
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False), "version": 2}
 
 
 def _copy_out(ptr, n: int, typestr: str, dtype) -> torch.Tensor:

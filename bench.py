@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- times the whole near-field hot path (nf_bin + nf_accel, all SURVEY.md 8(a) rows) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference] [--per-config LIST]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: nf_bin (cell ids, histogram,
+prefix sums, stable sort, gather, scheduling) followed by nf_accel (direct sum + scatter to input order).
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "near_field_pair_interactions_per_s"
+UNIT = "interactions/s"
+FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
+L2_BYTES = 126 * 1024 * 1024
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); default 3 = uniform 256^3")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--per-config", default="1,2,4", help="extra configs reported in 'per_config' (N=1 only); '' = none")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", type=int, default=None)
+    ap.add_argument("--fastpath", type=int, default=None)
+    ap.add_argument("--heavy-first", type=int, default=None)
+    ap.add_argument("--ctas-per-sm", type=int, default=None)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self.period = period
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "hw_power_brake_slowdown": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_min_mhz": min(self.samples), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------ oracle leg
+def oracle_sample_rate(pos_np, cfg, target_s=12.0):
+    """Times the oracle as it stands on a bounded sink sample of this workload (about target_s of CPU work).
+    Returns (interactions/s, description, seconds, cores)."""
+    import numpy as np
+    import oracle
+    t0 = time.time()
+    b = oracle.bin_particles(pos_np, cfg.cpd, cfg.L)
+    t_bin = time.time() - t0
+    rng = np.random.default_rng(12345)
+    n = pos_np.shape[0]
+    cnt = b["count"].astype(np.int64).reshape(cfg.cpd, cfg.cpd, cfg.cpd)
+    box = np.zeros_like(cnt)
+    R = cfg.R
+    for ox in range(-R, R + 1):
+        for oy in range(-R, R + 1):
+            for oz in range(-R, R + 1):
+                box += np.roll(cnt, (ox, oy, oz), axis=(0, 1, 2))
+    per_sink = box.reshape(-1)[b["cid"]]                   # sources per sink
+    # pilot to get the rate, then size the sample
+    pilot = rng.choice(n, size=min(n, 2000), replace=False)
+    t0 = time.time()
+    oracle.accel(pos_np, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=pilot, binning=b)
+    dt = max(time.time() - t0, 1e-4)
+    rate = per_sink[pilot].sum() / dt
+    want = rate * target_s
+    m = int(min(n, max(2000, want / max(per_sink.mean(), 1.0))))
+    sinks = rng.choice(n, size=m, replace=False)
+    t0 = time.time()
+    oracle.accel(pos_np, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=sinks, binning=b)
+    dt = time.time() - t0
+    inter = int(per_sink[sinks].sum())
+    desc = (f"{m} random sinks of {cfg.name} (all {n} particles binned by the oracle in {t_bin:.1f}s, "
+            f"{inter:.3e} pair interactions summed in {dt:.1f}s)")
+    return inter / dt, desc, dt, oracle.num_threads(), inter, m
+
+
+# ------------------------------------------------------------------------------------ GPU arm
+def fp32_peak_tflops(stats):
+    """SM count x 128 lanes x 2 flops x max SM clock, read from the device (BASELINE.json north_star)."""
+    return stats["sm_count"] * 128 * 2 * stats["clock_khz"] * 1e3 / 1e12
+
+
+def apply_options(plan, args):
+    for key, val in (("variant", args.variant), ("fastpath", args.fastpath), ("heavy_first", args.heavy_first),
+                     ("ctas_per_sm", args.ctas_per_sm)):
+        if val is not None:
+            plan.set_option(key, val)
+
+
+def time_device_steps(plan, pos, acc, steps, warmup, flush, dist=None):
+    """W warm-up steps, then exactly K timed steps between barrier + synchronize on both sides.
+    Returns (total_ms, [accel_ms per step], [bin_ms per step])."""
+    import torch
+    for _ in range(warmup):
+        plan.bin(pos)
+        plan.accel(acc)
+    torch.cuda.synchronize()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(steps):
+        if flush is not None:
+            flush.add_(1)                      # > L2 bytes written between iterations
+        ev[k][0].record()
+        plan.bin(pos)
+        ev[k][1].record()
+        plan.accel(acc)
+        ev[k][2].record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    bin_ms = [e[0].elapsed_time(e[1]) for e in ev]
+    acc_ms = [e[1].elapsed_time(e[2]) for e in ev]
+    total = sum(bin_ms) + sum(acc_ms)          # excludes the L2 flush writes, includes every kernel of the path
+    return total, acc_ms, bin_ms
+
+
+def time_e2e_steps(plan, pos_host, acc_host, steps, warmup):
+    """Same metric through the C-ABI with HOST (pinned) buffers: H2D of the positions and D2H of the
+    accelerations are inside every timed step.  Wall clock around synchronous calls (nf_accel_host syncs)."""
+    import torch
+    for _ in range(max(1, min(warmup, 2))):
+        plan.bin_host(pos_host)
+        plan.accel_host(acc_host)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        plan.bin_host(pos_host)
+        plan.accel_host(acc_host)
+    torch.cuda.synchronize()
+    return (time.perf_counter() - t0) * 1e3
+
+
+def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, warmup=None):
+    import torch
+    import nf_inputs
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.config(idx)
+    steps = steps or args.steps
+    warmup = warmup if warmup is not None else args.warmup
+    gen_dev = "cuda" if cfg.n > 20_000_000 else "cpu"
+    pos = nf_inputs.generate(cfg, device=gen_dev).cuda()
+    acc = torch.empty_like(pos)
+    input_bytes = pos.numel() * 4
+    flush = None
+    if input_bytes * 3 < 2 * L2_BYTES:         # small configs: flush L2 between timed iterations
+        flush = torch.zeros(2 * L2_BYTES // 4, dtype=torch.int32, device="cuda")
+    out = {"name": cfg.name, "n": cfg.n, "cpd": cfg.cpd}
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        apply_options(plan, args)
+        with ClockSampler(device_index) as clk:
+            total_ms, acc_ms, bin_ms = time_device_steps(plan, pos, acc, steps, warmup, flush, dist)
+        st = plan.stats()
+        out["clocks"] = clk.summary()
+        I = st["interactions"]
+        out.update(stats=st, interactions=I, total_ms=total_ms, accel_ms=acc_ms, bin_ms=bin_ms, steps=steps,
+                   l2="flushed between iterations (256 MiB write)" if flush is not None else "inputs exceed L2")
+        a = acc.double()
+        out["sum_check"] = float((a.sum(0).abs().max() / a.abs().sum()).item())   # total force ~ 0 at any size
+        if with_e2e:
+            pos_h = pos.cpu().pin_memory()
+            acc_h = torch.empty_like(pos_h).pin_memory()
+            e_steps = max(1, min(steps, 3))
+            out["e2e_ms"] = time_e2e_steps(plan, pos_h, acc_h, e_steps, warmup)
+            out["e2e_steps"] = e_steps
+            out["pos_host"] = pos_h
+    del pos, acc
+    torch.cuda.empty_cache()
+    return out, cfg
+
+
+def summarise(r):
+    st = r["stats"]
+    I, n = r["interactions"], r["n"]
+    t = r["total_ms"] / 1e3 / r["steps"]
+    ta = statistics.mean(r["accel_ms"]) / 1e3
+    peak = fp32_peak_tflops(st)
+    return {
+        "workload": r["name"], "n": n, "interactions": I,
+        "interactions_per_s": I / t, "particle_updates_per_s": n / t,
+        "accel_only_interactions_per_s": I / ta,
+        "ms_per_step": t * 1e3, "ms_bin": statistics.mean(r["bin_ms"]), "ms_accel": ta * 1e3,
+        "fp32_peak_frac_25flop": FLOPS_PER_INTERACTION * I / ta / 1e12 / peak,
+        "fp32_peak_frac_26flop_paper": 26 * I / ta / 1e12 / peak,
+        "sum_check": r["sum_check"], "l2": r["l2"], "clocks": r["clocks"],
+    }
+
+
+def main_b200(args):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    r, cfg = run_config(args.config, args, local, dist)
+    st = r["stats"]
+    t_total = r["total_ms"]
+    e2e_ms = r["e2e_ms"]
+    if dist is not None:                       # max over ranks: replicas only, no data-path collective
+        tt = torch.tensor([t_total, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_total, e2e_ms = tt.tolist()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    s = summarise(r)
+    I, n, K = r["interactions"], r["n"], r["steps"]
+    value = world * I * K / (t_total / 1e3)
+    ta = statistics.mean(r["accel_ms"]) / 1e3
+    peak = fp32_peak_tflops(st)
+    achieved = FLOPS_PER_INTERACTION * I / ta / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": t_total / K, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "n": n, "cpd": cfg.cpd, "R": cfg.R, "eps": cfg.eps, "L": cfg.L,
+                   "interactions_per_step": I, "l2": r["l2"], "multi_gpu": "replicas only (no collective)",
+                   "flops_per_interaction": FLOPS_PER_INTERACTION},
+        "particle_updates_per_s": world * n * K / (t_total / 1e3),
+        "fp32_peak_frac": s["fp32_peak_frac_25flop"], "fp32_peak_frac_26flop_paper": s["fp32_peak_frac_26flop_paper"],
+        "ms_bin": s["ms_bin"], "ms_accel": s["ms_accel"],
+        "e2e": {"value": world * I * r["e2e_steps"] / (e2e_ms / 1e3), "unit": UNIT, "h2d_bytes_per_step": 12 * n,
+                "d2h_bytes_per_step": 12 * n, "steps": r["e2e_steps"], "ms_per_step": e2e_ms / r["e2e_steps"],
+                "api": "nf_bin_host + nf_accel_host (pinned host buffers)"},
+        "gpu_launches": K * (st["kernel_launches_bin"] + st["kernel_launches_accel"]),
+        "clocks": r["clocks"],
+        "roofline": {"bound": "alu", "kernel": "nf::direct_kernel<packed f32x2>", "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": "SM count x 128 FP32 lanes x 2 x max SM clock read from the device (DESIGN.md)",
+                     "sm_count": st["sm_count"], "clock_khz": st["clock_khz"], "launch_ms": ta * 1e3,
+                     "grid": st["accel_grid"], "block": st["accel_block"]},
+        "sum_check": r["sum_check"],
+    }
+    if r["clocks"].get("sm_mhz"):
+        line["roofline"]["frac_at_sampled_clock"] = achieved / (peak * r["clocks"]["sm_mhz"] * 1e3 / st["clock_khz"])
+    if not args.no_cpu_baseline and world == 1:
+        v, desc, dt, cores, _, _ = oracle_sample_rate(r["pos_host"].numpy(), cfg)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    r.pop("pos_host", None)
+    if world == 1 and args.per_config:
+        per = [s]
+        for idx in [int(t) for t in args.per_config.split(",") if t]:
+            if idx == args.config:
+                continue
+            rr, _ = run_config(idx, args, local, None, with_e2e=False, steps=3, warmup=3)
+            per.append(summarise(rr))
+        line["per_config"] = per
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main_reference(args):
+    """The reference arm of this tier is the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import nf_inputs
+    cfg = nf_inputs.config(args.config)
+    import torch
+    dev = "cuda" if (cfg.n > 20_000_000 and torch.cuda.is_available()) else "cpu"
+    pos = nf_inputs.generate(cfg, device=dev).cpu().numpy()
+    per_step_target = max(2.0, min(12.0, 100.0 / (args.steps + args.warmup)))
+    rates, inter_tot, t_tot, desc, cores = [], 0, 0.0, "", 1
+    for k in range(args.warmup + args.steps):
+        v, desc, dt, cores, inter, m = oracle_sample_rate(pos, cfg, target_s=per_step_target)
+        if k >= args.warmup:
+            inter_tot += inter
+            t_tot += dt
+    value = inter_tot / t_tot
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_tot / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n": cfg.n, "cpd": cfg.cpd, "R": cfg.R, "eps": cfg.eps, "L": cfg.L},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "each step: " + desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        main_reference(a)
+    else:
+        main_b200(a)

@@ -36,7 +36,8 @@ size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells)
     const size_t C = ncells;
     const size_t nonempty = N < C ? N : C;
     const size_t pmax = N + 3 * nonempty + 8;
-    const size_t umax = nonempty + N / kChunk + 2;
+    const size_t ncol = (size_t)std::llround(std::cbrt((double)C)) * (size_t)std::llround(std::cbrt((double)C));
+    const size_t umax = (N < ncol ? N : ncol) + N / kChunk + 2;    // every column ends with one ragged window
     const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
     const size_t sort_blocks = (nsort + kSortTile - 1) / kSortTile + 1;
     const size_t scan_items = (256 * sort_blocks > C + 2 ? 256 * sort_blocks : C + 2);
@@ -50,6 +51,7 @@ size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells)
     ws.offset = (uint32_t *)take(4 * (C + 2));
     ws.poff   = (uint32_t *)take(4 * (C + 2));
     ws.ubase  = (uint32_t *)take(4 * (C + 2));
+    ws.src    = (uint32_t *)take(4 * (C + 1));
     ws.scan_tmp = (uint32_t *)take(4 * (scan_items / 2048 + 4096));
     ws.x = (float *)take(4 * pmax);
     ws.y = (float *)take(4 * pmax);

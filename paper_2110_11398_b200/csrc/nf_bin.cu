@@ -50,7 +50,6 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *t
 // ---- three-kernel exclusive scan with an element transform -----------------------------------
 struct OpId    { __device__ uint32_t operator()(uint32_t v) const { return v; } };
 struct OpPad4  { __device__ uint32_t operator()(uint32_t v) const { return (v + 3u) & ~3u; } };
-struct OpUnits { __device__ uint32_t operator()(uint32_t v) const { return (v + kChunk - 1) / kChunk; } };
 
 constexpr int kScanThreads = 256, kScanItems = 8, kScanTile = kScanThreads * kScanItems;
 
@@ -241,44 +240,33 @@ __global__ void __launch_bounds__(256) gather_kernel(const float *__restrict__ p
     }
 }
 
-// ---- S5: work units, cost keys, exact interaction count ------------------------------------------------------
-__global__ void __launch_bounds__(256) units_kernel(Consts k, const uint32_t *__restrict__ count,
-                                                    const uint32_t *__restrict__ ubase, Unit *__restrict__ units,
-                                                    uint32_t *__restrict__ ukey, unsigned long long *__restrict__ interactions)
+// ---- S5: stencil source counts, work units, cost keys, exact interaction count -------------------------------
+// src[c] = particles in the (2R+1)^3 periodic stencil of cell c; interactions = sum_c count[c] * src[c].
+__global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t *__restrict__ count,
+                                                       uint32_t *__restrict__ src_out,
+                                                       unsigned long long *__restrict__ interactions)
 {
     __shared__ unsigned long long red[8];
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long mine = 0;
     if (c < k.ncells) {
-        const uint32_t nc = count[c];
-        if (nc) {
-            const int cpd = k.cpd, R = k.R;
-            const int cz = c % cpd, cy = (c / cpd) % cpd, cx = c / (cpd * cpd);
-            unsigned long long src = 0;
-            for (int ox = -R; ox <= R; ox++) {
-                int sx = cx + ox; sx += sx < 0 ? cpd : 0; sx -= sx >= cpd ? cpd : 0;
-                for (int oy = -R; oy <= R; oy++) {
-                    int sy = cy + oy; sy += sy < 0 ? cpd : 0; sy -= sy >= cpd ? cpd : 0;
-                    for (int oz = -R; oz <= R; oz++) {
-                        int sz = cz + oz; sz += sz < 0 ? cpd : 0; sz -= sz >= cpd ? cpd : 0;
-                        src += count[((uint32_t)sx * cpd + sy) * cpd + sz];
-                    }
+        const int cpd = k.cpd, R = k.R;
+        const int cz = c % cpd, cy = (c / cpd) % cpd, cx = c / (cpd * cpd);
+        uint32_t src = 0;                        // <= n < 2^32
+        for (int ox = -R; ox <= R; ox++) {
+            int sx = cx + ox; sx += sx < 0 ? cpd : 0; sx -= sx >= cpd ? cpd : 0;
+            for (int oy = -R; oy <= R; oy++) {
+                int sy = cy + oy; sy += sy < 0 ? cpd : 0; sy -= sy >= cpd ? cpd : 0;
+                const uint32_t row = ((uint32_t)sx * cpd + sy) * cpd;
+                for (int oz = -R; oz <= R; oz++) {
+                    int sz = cz + oz; sz += sz < 0 ? cpd : 0; sz -= sz >= cpd ? cpd : 0;
+                    src += count[row + sz];
                 }
             }
-            mine = (unsigned long long)nc * src;
-            const uint32_t ub = ubase[c];
-            const uint32_t nu = (nc + kChunk - 1) / kChunk;
-            for (uint32_t u = 0; u < nu; u++) {
-                Unit un;
-                un.cell = c; un.k0 = u * kChunk;
-                un.nk = nc - un.k0 < (uint32_t)kChunk ? nc - un.k0 : (uint32_t)kChunk;
-                un.cost_hi = src > 0xffffffffull ? 0xffffffffu : (uint32_t)src;
-                units[ub + u] = un;
-                ukey[ub + u] = (uint32_t)__clzll((long long)((unsigned long long)un.nk * src));   // heavier -> smaller key
-            }
         }
+        src_out[c] = src;
+        mine = (unsigned long long)count[c] * src;
     }
-    // block reduction of the interaction count
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(0xffffffffu, mine, o);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mine;
@@ -287,6 +275,48 @@ __global__ void __launch_bounds__(256) units_kernel(Consts k, const uint32_t *__
         unsigned long long t = 0;
         for (int w = 0; w < 8; w++) t += red[w];
         if (t) atomicAdd(interactions, t);
+    }
+}
+
+// work units per z-column: windows of kChunk consecutive cell-sorted sinks
+__global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ offset,
+                                                       uint32_t *__restrict__ nunits)
+{
+    const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= (uint32_t)(k.cpd * k.cpd)) return;
+    const uint32_t ncol = offset[(size_t)(col + 1) * k.cpd] - offset[(size_t)col * k.cpd];
+    nunits[col] = (ncol + kChunk - 1) / kChunk;
+}
+
+// One thread per column walks its cells once and emits the column's units with their cost keys.
+__global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ offset,
+                                                    const uint32_t *__restrict__ src, const uint32_t *__restrict__ ubase,
+                                                    Unit *__restrict__ units, uint32_t *__restrict__ ukey)
+{
+    const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= (uint32_t)(k.cpd * k.cpd)) return;
+    const uint32_t *off = offset + (size_t)col * k.cpd;
+    const uint32_t *sc = src + (size_t)col * k.cpd;
+    const uint32_t c_begin = off[0], c_end = off[k.cpd];
+    uint32_t u = ubase[col];
+    int z = 0;
+    for (uint32_t s0 = c_begin; s0 < c_end; s0 += kChunk, u++) {
+        const uint32_t s1 = min(s0 + (uint32_t)kChunk, c_end);
+        while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
+        Unit un;
+        un.s0 = s0; un.col = col; un.ns = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
+        unsigned long long cost = 0;
+        int zz = z;
+        for (;;) {
+            const uint32_t lo = max(off[zz], s0), hi = min(off[zz + 1], s1);
+            cost += (unsigned long long)(hi - lo) * sc[zz];
+            if (off[zz + 1] >= s1) break;
+            zz++;
+        }
+        un.z1 = (uint16_t)zz;
+        units[u] = un;
+        ukey[u] = (uint32_t)__clzll((long long)cost);     // heavier -> smaller key
+        z = zz;
     }
 }
 
@@ -320,7 +350,6 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     // prefix sums: offset (exported), padded offsets, unit bases
     exclusive_scan(ws.count, ws.offset, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
     exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
-    exclusive_scan(ws.count, ws.ubase, (size_t)k.ncells, ws.scan_tmp, OpUnits(), 1, &ws.scalars[2], st, &L);
 
     // stable sort by cell id
     int bits = 1;
@@ -338,12 +367,17 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 
     gather_kernel<<<nb256, 256, 0, st>>>(pos, n, k, p->sorted_keys, p->perm, ws.offset, ws.poff, ws.x, ws.y, ws.z);  L++;
 
-    // units + heavy-first order: one stable radix pass on the cost key (clz of the unit's interaction
-    // count, so heavier units come first and equal keys keep cell order).  The keys sit in the storage
-    // of units_sorted until the order is known; the sort writes into the free particle-sort buffers.
+    // stencil source counts + exact interaction count, units per column, units + heavy-first order: one
+    // stable radix pass on the cost key (clz of the unit's interaction count, so heavier units come first
+    // and equal keys keep column order).  The keys sit in the storage of units_sorted until the order is
+    // known; the sort writes into the free particle-sort buffers.
     const unsigned nbc = (k.ncells + 255) / 256;
+    const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
     uint32_t *ukey = (uint32_t *)ws.units_sorted;
-    units_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.ubase, ws.units, ukey, ws.interactions);  L++;
+    cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions);  L++;
+    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.offset, ws.ubase);  L++;
+    exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
+    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.offset, ws.src, ws.ubase, ws.units, ukey);  L++;
     NF_CUDA_OK(cudaGetLastError());
 
     // domain flag + unit count: the one documented synchronisation of nf_bin

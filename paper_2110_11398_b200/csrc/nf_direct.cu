@@ -5,18 +5,26 @@
 //   O(N^2) summation with a compact spline softening kernel"; periodic images kept).
 //
 // Design (sm_100a):
-//   * persistent CTAs, one producer warp + kConsumerWarps consumer warps, work units (<= 128 sinks of one
-//     cell) pulled from an atomic counter in heavy-first order;
-//   * the producer streams each of the (2R+1)^2 z-pencils of the stencil into shared memory with TMA 1-D
-//     bulk copies (cp.async.bulk + mbarrier complete_tx) through a kStages-deep ring; consumers never touch
-//     global memory in the pair loop;
-//   * one sink per lane in registers; sources are read as broadcast LDS.128 of 4 x, 4 y, 4 z and processed as
-//     two packed pairs with FFMA2/FADD2/FMUL2 (fma.rn.f32x2), one MUFU.RSQ per interaction;
-//   * coordinates are cell-corner relative (exact), the periodic wrap is a per-(sink cell, source cell)
-//     constant subtracted from the sink once per piece -- nothing periodic in the pair loop;
+//   * a work unit is a WINDOW of <= kChunk consecutive cell-sorted sinks of one z-column (cells are z-fastest,
+//     so a column is one contiguous run of the sorted order): every warp holds 32 real sinks whatever the
+//     cell occupancy -- no lane is lost to the ~68-particles-per-cell granularity;
+//   * persistent CTAs, one producer warp + kConsumerWarps consumer warps, units pulled from an atomic
+//     counter in heavy-first order;
+//   * for each of the (2R+1)^2 neighbour columns the producer streams the z-run of cells [z0-R, z1+R] that the
+//     window's sinks need into shared memory with TMA 1-D bulk copies (cp.async.bulk + mbarrier complete_tx)
+//     through a kStages-deep ring, with a table of the cells (pieces) of the run;
+//   * a lane whose sink sits in cell zc walks ITS OWN 2R+1 pieces zc-R..zc+R of the run: in step t every
+//     lane of the warp reads the piece at offset t-R from its own cell, so lanes of different cells read
+//     different pieces in the same instruction (per-lane shared-memory pointer, one LDS.128 wavefront per
+//     distinct cell) and no lane ever evaluates a pair outside its stencil;
+//   * one sink per lane in registers; sources are read as LDS.128 of 4 x, 4 y, 4 z and processed as two
+//     packed pairs with FFMA2/FADD2/FMUL2 (fma.rn.f32x2), one MUFU.RSQ per interaction;
+//   * coordinates are cell-corner relative (exact); the periodic wrap and the cell-to-cell shift are one
+//     constant per (sink cell, source cell) subtracted from the sink once per piece -- nothing periodic
+//     in the pair loop;
 //   * cells whose max-norm offset is >= 2 cannot hold a pair closer than eps_s (when eps_s <= cell width):
 //     they take the pure Newtonian body (no spline, no min);
-//   * FP32 FMA chain per (sink, source cell) piece, piece partials added in FP64 (two-level accumulation);
+//   * FP32 FMA chain per (sink, stage), stage partials added in FP64 (two-level accumulation);
 //   * the epilogue writes acc[perm[s]] directly (S7 fused, no sorted acceleration buffer).
 #include "nf_internal.h"
 
@@ -24,27 +32,28 @@ namespace nf {
 
 enum { kFlagBegin = 1, kFlagEnd = 2, kFlagTerm = 4 };
 
-struct Piece {          // one source cell (or part of one) inside a stage
-    int   sm_off;       // first slot in the stage buffers (multiple of 4)
-    int   nslots;       // multiple of 4
-    float dx, dy, dz;   // sink shift: d = x_src - (x_sink - shift), scaled cell-relative units
-    int   soft;         // 1: spline + min body, 0: pure Newtonian body
+struct __align__(16) Piece {   // one source cell (or a part of one) of the stage's z-run
+    int    sm_off;             // first slot in the stage buffers (multiple of 4)
+    int    nslots;             // multiple of 4; 0 = empty cell
+    double czs;                // (corner_z(source cell) + box wrap) * scale
 };
 
-struct StageDesc {
+struct __align__(16) StageDesc {
     int      flags;
     int      npieces;
-    uint32_t sink_p0;   // padded slot of the unit's first sink
-    uint32_t nsink;
-    uint32_t out0;      // sorted (unpadded) slot of the unit's first sink -> perm index
-    int      pad_[3];
+    int      j0;               // cell of pieces[0], as an index relative to z0 - R
+    int      soft_mode;        // 2: spline body everywhere; 1: for |oz| <= 1 (column with |ox|,|oy| <= 1); 0: never
+    float    dx, dy;           // sink shift of this column: d = x_src - (x_sink - shift), scaled units
+    uint32_t s0;               // unit: first sorted slot
+    uint32_t ns;               //       sinks
+    uint32_t z0, z1;           //       first / last sink cell (z index)
+    uint32_t colbase;          //       col * cpd
+    int      pad_;
     Piece    pieces[kMaxPieces];
 };
 
 struct __align__(128) SharedStorage {
-    float sx[kStages][kTile];
-    float sy[kStages][kTile];
-    float sz[kStages][kTile];
+    float buf[kStages][3][kTile];      // x, y, z of the staged sources
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
@@ -135,37 +144,40 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
     az = fmaf(k, dz, az);
 }
 
+// FP32 partial sums of one (sink, stage): two chains per component (packed: the two halves of an f32x2)
+struct Partial {
+    float2 x, y, z;
+    __device__ __forceinline__ void clear() { x = y = z = make_float2(0.f, 0.f); }
+};
+
 template <bool PACKED, bool SOFT>
-__device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const float4 *__restrict__ py,
-                                           const float4 *__restrict__ pz, const int n4, const float sxi, const float syi,
-                                           const float szi, const SoftCoef &c, double &ax, double &ay, double &az)
+__device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float sxi, const float syi,
+                                     const float szi, const SoftCoef &c, Partial &f)
 {
     if (PACKED) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        float2 fx = make_float2(0.f, 0.f), fy = fx, fz = fx;
-#pragma unroll 2
-        for (int j = 0; j < n4; j++) {
-            const float4 X = px[j], Y = py[j], Z = pz[j];
-            interact2<SOFT>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, fx, fy, fz);
-            interact2<SOFT>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, fx, fy, fz);
-        }
-        ax += (double)fx.x + (double)fx.y;
-        ay += (double)fy.x + (double)fy.y;
-        az += (double)fz.x + (double)fz.y;
+        interact2<SOFT>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2<SOFT>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
     } else {
-        float fx0 = 0.f, fy0 = 0.f, fz0 = 0.f, fx1 = 0.f, fy1 = 0.f, fz1 = 0.f;
-#pragma unroll 2
-        for (int j = 0; j < n4; j++) {
-            const float4 X = px[j], Y = py[j], Z = pz[j];
-            interact1<SOFT>(X.x, Y.x, Z.x, sxi, syi, szi, c, fx0, fy0, fz0);
-            interact1<SOFT>(X.y, Y.y, Z.y, sxi, syi, szi, c, fx1, fy1, fz1);
-            interact1<SOFT>(X.z, Y.z, Z.z, sxi, syi, szi, c, fx0, fy0, fz0);
-            interact1<SOFT>(X.w, Y.w, Z.w, sxi, syi, szi, c, fx1, fy1, fz1);
-        }
-        ax += (double)fx0 + (double)fx1;
-        ay += (double)fy0 + (double)fy1;
-        az += (double)fz0 + (double)fz1;
+        interact1<SOFT>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x);
+        interact1<SOFT>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y);
+        interact1<SOFT>(X.z, Y.z, Z.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x);
+        interact1<SOFT>(X.w, Y.w, Z.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y);
     }
+}
+
+// One step of a warp: every lane runs over ITS piece (n4 quads at px); nmin / nmax are the warp's smallest and
+// largest n4, so the first loop is uniform and only the ragged tail is predicated per lane.
+template <bool PACKED, bool SOFT>
+__device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
+                                           const float sxi, const float syi, const float szi, const SoftCoef &c, Partial &f)
+{
+    const float4 *__restrict__ py = px + kTile / 4;
+    const float4 *__restrict__ pz = py + kTile / 4;
+#pragma unroll 2
+    for (int j = 0; j < nmin; j++) quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+    for (int j = nmin; j < nmax; j++)
+        if (j < n4) quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
 }
 
 // ---- the kernel --------------------------------------------------------------------------------
@@ -180,139 +192,185 @@ struct AccelArgs {
     int fastpath;
 };
 
-template <bool PACKED>
-__global__ void __launch_bounds__(kAccelThreads) direct_kernel(const AccelArgs a)
+constexpr uint32_t kFull = 0xffffffffu;
+
+// The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
+// descriptors, the barriers and the TMA unit.
+__device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, const int lane)
 {
-    __shared__ SharedStorage sm;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-
-    if (tid == 0) {
-        for (int s = 0; s < kStages; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kConsumerWarps); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-
-    if (warp == kConsumerWarps) {
-        // ================================ producer (one lane) ================================
-        if (lane != 0) return;
-        const Consts &k = a.k;
-        const int cpd = k.cpd, R = k.R;
-        int stage = 0;
-        uint32_t phase = 0;
-        bool open = false, sealed = false;
-        int fill = 0, np = 0, sflags = 0;
-        // pending merged copy
-        uint32_t cp_g = 0, cp_s = 0, cp_n = 0;
-        auto flush_copy = [&]() {
-            if (cp_n) {
-                tma_load_1d(&sm.sx[stage][cp_s], a.x + cp_g, cp_n * 4u, &sm.full[stage]);
-                tma_load_1d(&sm.sy[stage][cp_s], a.y + cp_g, cp_n * 4u, &sm.full[stage]);
-                tma_load_1d(&sm.sz[stage][cp_s], a.z + cp_g, cp_n * 4u, &sm.full[stage]);
-                cp_n = 0;
-            }
-        };
-        auto commit = [&](int extra) {
-            flush_copy();
+    const Consts &k = a.k;
+    const int cpd = k.cpd, R = k.R;
+    const bool lead = lane == 0;
+    int stage = 0;
+    uint32_t phase = 0;
+    bool open = false, sealed = false;
+    int fill = 0, np = 0, sflags = 0;
+    uint32_t cp_g = 0, cp_s = 0, cp_n = 0;        // pending merged copy: global slot, stage slot, slots
+    auto flush_copy = [&]() {
+        if (cp_n && lead) {
+            tma_load_1d(&sm.buf[stage][0][cp_s], a.x + cp_g, cp_n * 4u, &sm.full[stage]);
+            tma_load_1d(&sm.buf[stage][1][cp_s], a.y + cp_g, cp_n * 4u, &sm.full[stage]);
+            tma_load_1d(&sm.buf[stage][2][cp_s], a.z + cp_g, cp_n * 4u, &sm.full[stage]);
+        }
+        cp_n = 0;
+    };
+    auto commit = [&](int extra) {
+        flush_copy();
+        if (lead) {
             sm.desc[stage].flags = sflags | extra;
             sm.desc[stage].npieces = np;
             mbar_arrive_expect_tx(&sm.full[stage], (uint32_t)fill * 12u);
-            if (++stage == kStages) { stage = 0; phase ^= 1u; }
-            open = false; sealed = false;
-        };
-        for (;;) {
-            const uint32_t u = atomicAdd(a.counter, 1u);
-            if (u >= a.n_units) break;
-            const Unit un = a.units[u];
-            const int cz = un.cell % cpd, cy = (un.cell / cpd) % cpd, cx = un.cell / (cpd * cpd);
-            const uint32_t sink_p0 = __ldg(a.poff + un.cell) + un.k0;
-            const uint32_t out0 = __ldg(a.offset + un.cell) + un.k0;
-            const double ocx = (double)(float)((double)cx * k.cell_w), ocy = (double)(float)((double)cy * k.cell_w),
-                         ocz = (double)(float)((double)cz * k.cell_w);
-            bool first = true;
-            for (int ox = -R; ox <= R; ox++) {
-                int jx = cx + ox; double wx = 0.0;
-                if (jx < 0) { jx += cpd; wx = -k.L; } else if (jx >= cpd) { jx -= cpd; wx = k.L; }
-                const float Dx = (float)(((double)(float)((double)jx * k.cell_w) + wx - ocx) * k.scale);
-                for (int oy = -R; oy <= R; oy++) {
-                    int jy = cy + oy; double wy = 0.0;
-                    if (jy < 0) { jy += cpd; wy = -k.L; } else if (jy >= cpd) { jy -= cpd; wy = k.L; }
-                    const float Dy = (float)(((double)(float)((double)jy * k.cell_w) + wy - ocy) * k.scale);
-                    const uint32_t row = ((uint32_t)jx * cpd + jy) * cpd;
-                    for (int oz = -R; oz <= R; oz++) {
-                        int jz = cz + oz; double wz = 0.0;
-                        if (jz < 0) { jz += cpd; wz = -k.L; } else if (jz >= cpd) { jz -= cpd; wz = k.L; }
-                        uint32_t p0 = __ldg(a.poff + row + jz);
-                        const uint32_t p1 = __ldg(a.poff + row + jz + 1);
-                        if (p0 == p1) continue;
-                        const float Dz = (float)(((double)(float)((double)jz * k.cell_w) + wz - ocz) * k.scale);
-                        const int far = (ox > 1 || ox < -1 || oy > 1 || oy < -1 || oz > 1 || oz < -1);
-                        const int soft = !(far && k.fast_ok && a.fastpath);
-                        while (p0 < p1) {
-                            if (open && (sealed || fill == kTile)) commit(0);
+        }
+        if (++stage == kStages) { stage = 0; phase ^= 1u; }
+        open = false; sealed = false;
+    };
+    for (;;) {
+        uint32_t u = 0;
+        if (lead) u = atomicAdd(a.counter, 1u);
+        u = __shfl_sync(kFull, u, 0);
+        if (u >= a.n_units) break;
+        const Unit un = a.units[u];
+        const int cx = (int)(un.col / (uint32_t)cpd), cy = (int)(un.col % (uint32_t)cpd);
+        const int z0 = un.z0, z1 = un.z1;
+        const double ocx = (double)(float)((double)cx * k.cell_w), ocy = (double)(float)((double)cy * k.cell_w);
+        const int jlo = z0 - R, jhi = z1 + R;     // unwrapped z-run every neighbour column contributes
+        bool first = true;
+        for (int ox = -R; ox <= R; ox++) {
+            int jx = cx + ox; double wx = 0.0;
+            if (jx < 0) { jx += cpd; wx = -k.L; } else if (jx >= cpd) { jx -= cpd; wx = k.L; }
+            const float Dx = (float)(((double)(float)((double)jx * k.cell_w) + wx - ocx) * k.scale);
+            for (int oy = -R; oy <= R; oy++) {
+                int jy = cy + oy; double wy = 0.0;
+                if (jy < 0) { jy += cpd; wy = -k.L; } else if (jy >= cpd) { jy -= cpd; wy = k.L; }
+                const float Dy = (float)(((double)(float)((double)jy * k.cell_w) + wy - ocy) * k.scale);
+                const uint32_t row = ((uint32_t)jx * cpd + jy) * cpd;
+                const int soft_mode = !(k.fast_ok && a.fastpath) ? 2 : ((ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1) ? 1 : 0);
+                for (int jb = jlo; jb <= jhi; jb += 32) {
+                    // the warp fetches the padded offsets of up to 32 cells of the run at once
+                    const int jl = jb + lane;
+                    int jwl = jl;
+                    if (jwl < 0) jwl += cpd; else if (jwl >= cpd) jwl -= cpd;
+                    uint32_t P0 = 0, P1 = 0;
+                    if (jl <= jhi) { P0 = __ldg(a.poff + row + jwl); P1 = __ldg(a.poff + row + jwl + 1); }
+                    const int cnt = min(32, jhi - jb + 1);
+                    for (int q = 0; q < cnt; q++) {
+                        uint32_t p0 = __shfl_sync(kFull, P0, q);
+                        const uint32_t p1 = __shfl_sync(kFull, P1, q);
+                        const bool empty = p0 == p1;
+                        if (empty && (!open || sealed || fill == kTile || np == kMaxPieces)) continue;   // empty cells never open a stage
+                        const int j = jb + q;
+                        int jw = j; double wz = 0.0;
+                        if (jw < 0) { jw += cpd; wz = -k.L; } else if (jw >= cpd) { jw -= cpd; wz = k.L; }
+                        const double czs = ((double)(float)((double)jw * k.cell_w) + wz) * k.scale;
+                        do {
+                            if (open && (sealed || fill == kTile || np == kMaxPieces)) commit(0);
                             if (!open) {
+                                if (empty) break;
                                 mbar_wait(&sm.empty[stage], phase ^ 1u);
                                 open = true; fill = 0; np = 0;
                                 sflags = first ? kFlagBegin : 0;
                                 first = false;
-                                sm.desc[stage].sink_p0 = sink_p0;
-                                sm.desc[stage].nsink = un.nk;
-                                sm.desc[stage].out0 = out0;
+                                if (lead) {
+                                    StageDesc &d = sm.desc[stage];
+                                    d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy;
+                                    d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.colbase = un.col * (uint32_t)cpd;
+                                }
                             }
                             const uint32_t t = min(p1 - p0, (uint32_t)(kTile - fill));
-                            Piece &pc = sm.desc[stage].pieces[np++];
-                            pc.sm_off = fill; pc.nslots = (int)t; pc.dx = Dx; pc.dy = Dy; pc.dz = Dz; pc.soft = soft;
+                            if (lead) {
+                                Piece &pc = sm.desc[stage].pieces[np];
+                                pc.sm_off = fill; pc.nslots = (int)t; pc.czs = czs;
+                            }
+                            np++;
                             if (cp_n && cp_g + cp_n == p0 && cp_s + cp_n == (uint32_t)fill) cp_n += t;
                             else { flush_copy(); cp_g = p0; cp_s = (uint32_t)fill; cp_n = t; }
                             fill += (int)t; p0 += t;
-                        }
+                        } while (p0 < p1);
                     }
-                    if (open) sealed = true;      // one z-pencil per stage
                 }
+                if (open) sealed = true;          // one neighbour column per stage
             }
-            commit(kFlagEnd);                     // the own cell is never empty, so a stage is open
         }
-        mbar_wait(&sm.empty[stage], phase ^ 1u);
+        commit(kFlagEnd);                         // the sinks' own cells are never empty, so a stage is open
+    }
+    mbar_wait(&sm.empty[stage], phase ^ 1u);
+    if (lead) {
         sm.desc[stage].flags = kFlagTerm;
         sm.desc[stage].npieces = 0;
         mbar_arrive_expect_tx(&sm.full[stage], 0u);
-        return;
     }
+}
 
-    // ==================================== consumers ====================================
+template <bool PACKED>
+__device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
+{
     const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny};
+    const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;
     float xi = 0.f, yi = 0.f, zi = 0.f;
-    double ax = 0.0, ay = 0.0, az = 0.0;
-    uint32_t nsink = 0, out0 = 0;
+    double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0;
+    int zrel = 0;                       // the lane's sink cell, relative to z0
+    uint32_t slot = 0;                  // the lane's sorted slot (perm index)
+    bool act = false, warp_on = false;
     for (;;) {
         mbar_wait(&sm.full[stage], phase);
         const StageDesc &d = sm.desc[stage];
         const int flags = d.flags;
         if (flags & kFlagTerm) break;
         if (flags & kFlagBegin) {
-            nsink = d.nsink; out0 = d.out0;
-            const uint32_t p = d.sink_p0 + (uint32_t)tid;
-            const bool act = (uint32_t)tid < nsink;
-            xi = act ? __ldg(a.x + p) : 0.f;
-            yi = act ? __ldg(a.y + p) : 0.f;
-            zi = act ? __ldg(a.z + p) : 0.f;
+            const uint32_t ns = d.ns, kk = (uint32_t)(warp * 32 + lane);
+            warp_on = (uint32_t)(warp * 32) < ns;
+            act = kk < ns;
             ax = ay = az = 0.0;
-        }
-        if ((uint32_t)(warp * 32) < nsink) {
-            const int np = d.npieces;
-            for (int q = 0; q < np; q++) {
-                const Piece pc = d.pieces[q];
-                const float4 *px = reinterpret_cast<const float4 *>(&sm.sx[stage][pc.sm_off]);
-                const float4 *py = reinterpret_cast<const float4 *>(&sm.sy[stage][pc.sm_off]);
-                const float4 *pz = reinterpret_cast<const float4 *>(&sm.sz[stage][pc.sm_off]);
-                const float sxi = pc.dx - xi, syi = pc.dy - yi, szi = pc.dz - zi;   // -(x_i - shift)
-                if (pc.soft) piece_loop<PACKED, true>(px, py, pz, pc.nslots >> 2, sxi, syi, szi, coef, ax, ay, az);
-                else         piece_loop<PACKED, false>(px, py, pz, pc.nslots >> 2, sxi, syi, szi, coef, ax, ay, az);
+            if (warp_on) {
+                // lanes past the end of a ragged window shadow its last sink (same pieces, nothing written)
+                slot = d.s0 + (act ? kk : ns - 1u);
+                const uint32_t *off = a.offset + d.colbase;
+                int lo = (int)d.z0, hi = (int)d.z1;
+                while (lo < hi) {                      // last cell of [z0, z1] whose first slot is <= slot
+                    const int mid = (lo + hi + 1) >> 1;
+                    if (__ldg(off + mid) <= slot) lo = mid; else hi = mid - 1;
+                }
+                zrel = lo - (int)d.z0;
+                const uint32_t p = __ldg(a.poff + d.colbase + lo) + (slot - __ldg(off + lo));
+                xi = __ldg(a.x + p); yi = __ldg(a.y + p); zi = __ldg(a.z + p);
+                oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
             }
         }
-        if ((flags & kFlagEnd) && (uint32_t)tid < nsink) {
-            const size_t i = __ldg(a.perm + out0 + tid);
+        if (warp_on) {
+            const int np = d.npieces, soft_mode = d.soft_mode;
+            const float sxi = d.dx - xi, syi = d.dy - yi;           // -(x_i - shift)
+            const int ibase = zrel - d.j0;
+            const float4 *sbase = reinterpret_cast<const float4 *>(&sm.buf[stage][0][0]);
+            Partial f;
+            f.clear();
+            for (int t = 0; t < nsteps; t++) {
+                const int idx = ibase + t;                          // the lane's piece for cell zc - R + t
+                const bool valid = (unsigned)idx < (unsigned)np;
+                int n4 = 0, sm_off = 0;
+                double czs = 0.0;
+                if (valid) {
+                    const Piece pc = d.pieces[idx];
+                    n4 = pc.nslots >> 2; sm_off = pc.sm_off; czs = pc.czs;
+                }
+                const int nmax = __reduce_max_sync(kFull, n4);
+                if (nmax == 0) continue;
+                const int nmin = __reduce_min_sync(kFull, n4);
+                const float szi = (float)(czs - oczs) - zi;
+                const float4 *px = sbase + (sm_off >> 2);
+                const int dt = t - R;
+                const bool soft = soft_mode == 2 || (soft_mode == 1 && dt >= -1 && dt <= 1);
+                if (soft) piece_loop<PACKED, true>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
+                else      piece_loop<PACKED, false>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
+            }
+            ax += (double)f.x.x + (double)f.x.y;
+            ay += (double)f.y.x + (double)f.y.y;
+            az += (double)f.z.x + (double)f.z.y;
+        }
+        if ((flags & kFlagEnd) && act) {
+            const size_t i = __ldg(a.perm + slot);
             const double s2 = a.k.out_scale;
             a.acc[3 * i + 0] = (float)(ax * s2);
             a.acc[3 * i + 1] = (float)(ay * s2);
@@ -322,6 +380,20 @@ __global__ void __launch_bounds__(kAccelThreads) direct_kernel(const AccelArgs a
         if (lane == 0) mbar_arrive(&sm.empty[stage]);
         if (++stage == kStages) { stage = 0; phase ^= 1u; }
     }
+}
+
+template <bool PACKED>
+__global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
+{
+    __shared__ SharedStorage sm;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        for (int s = 0; s < kStages; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kConsumerWarps); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == kConsumerWarps) producer(a, sm, lane);
+    else                        consumer<PACKED>(a, sm, warp, lane);
 }
 
 int accel_max_ctas_per_sm(int variant)

@@ -11,13 +11,26 @@
 namespace nf {
 
 // ---- compile-time shape of the direct-sum kernel -------------------------------------------
-constexpr int kMaxR          = 4;                 // (2R+1) <= 9 pieces per stage
-constexpr int kMaxPieces     = 2 * kMaxR + 1;
-constexpr int kConsumerWarps = 4;                 // sink lanes per CTA = 128
-constexpr int kChunk         = 32 * kConsumerWarps;   // sinks per work unit
-constexpr int kTile          = 512;               // source slots per pipeline stage (multiple of 4)
-constexpr int kStages        = 3;                 // TMA pipeline depth
+constexpr int kMaxR          = 4;                 // stencil (2R+1)^3 with R <= 4
+#ifndef NF_CONSUMER_WARPS
+#define NF_CONSUMER_WARPS 4
+#endif
+#ifndef NF_TILE
+#define NF_TILE 768
+#endif
+#ifndef NF_STAGES
+#define NF_STAGES 3
+#endif
+#ifndef NF_MIN_CTAS
+#define NF_MIN_CTAS 6
+#endif
+constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // sink lanes per CTA = 32 * kConsumerWarps
+constexpr int kChunk         = 32 * kConsumerWarps;   // max sinks per work unit (a window of one z-column)
+constexpr int kTile          = NF_TILE;           // source slots per pipeline stage (multiple of 4)
+constexpr int kStages        = NF_STAGES;         // TMA pipeline depth
+constexpr int kMaxPieces     = 24;                // source cells (table entries) per stage
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
+constexpr int kMinCtasPerSm  = NF_MIN_CTAS;       // register budget: 65536 / (kMinCtasPerSm * kAccelThreads) per thread
 constexpr float kDummy       = 36028797018963968.0f;        // 2^55: pad-slot coordinate, contributes exactly 0
 
 // ---- radix sort shape ----------------------------------------------------------------------
@@ -26,17 +39,19 @@ constexpr int kSortThreads = 32 * kSortWarps;
 constexpr int kSortItems   = 16;                          // keys per thread
 constexpr int kSortTile    = kSortThreads * kSortItems;   // 4096 keys per block
 
-struct Unit {            // one work unit: a chunk of <= kChunk sinks of one cell
-    uint32_t cell;
-    uint32_t k0;         // first sink within the cell
-    uint32_t nk;         // sinks in the chunk
-    uint32_t cost_hi;    // Sum of stencil counts (sources per sink), saturated
+struct Unit {            // one work unit: a window of <= kChunk consecutive cell-sorted sinks of one z-column
+    uint32_t s0;         // first sorted slot (index into perm)
+    uint32_t col;        // column id cx * cpd + cy
+    uint16_t ns;         // sinks in the window
+    uint16_t z0, z1;     // first and last cell (z index) that hold a sink of the window
+    uint16_t pad_;
 };
 
 struct Workspace {       // carved out of one arena; all 256-byte aligned
     uint32_t *cid, *keyA, *keyB, *valA, *valB;   // [n]
     uint32_t *radix_hist;                         // [256 * sort_blocks]
-    uint32_t *count, *offset, *poff, *ubase;      // [C], [C+1], [C+1], [C+1]
+    uint32_t *count, *offset, *poff, *ubase;      // [C], [C+1], [C+1], [cpd^2+1] (unit base per column)
+    uint32_t *src;                                // [C] particles in the stencil of each cell
     uint32_t *scan_tmp;                           // block sums
     float *x, *y, *z;                             // [P_max]
     Unit *units, *units_sorted;                   // [U_max]

@@ -164,6 +164,12 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
         k.A = (float)A; k.B = (float)B; k.C = (float)C;
     }
     k.fast_ok = (2.16 * eps <= 0.999 * k.cell_w) ? 1 : 0;
+    k.w_scaled = (float)(k.cell_w * k.scale);
+    {   // cell-relative coordinates carry the float32 rounding of the position and of the corner: <= 2^-23 L each
+        const double margin = 4.0 * 1.2e-7 * L * k.scale;
+        const double thr = es + margin;
+        k.soft_thr2 = (float)(thr * thr * 1.0001);
+    }
     p->eps = eps;
     p->device = -1;
     p->stream = 0;

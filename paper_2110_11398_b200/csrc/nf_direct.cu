@@ -48,7 +48,7 @@ struct __align__(16) StageDesc {
     uint32_t ns;               //       sinks
     uint32_t z0, z1;           //       first / last sink cell (z index)
     uint32_t colbase;          //       col * cpd
-    int      pad_;
+    int      oxy;              // column offset: (ox + 8) | (oy + 8) << 8
     Piece    pieces[kMaxPieces];
 };
 
@@ -71,8 +71,9 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
     const uint32_t a = smem_u32(bar);
     uint32_t ok;
     do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        // the suspend-time hint parks the warp in hardware instead of spinning through issue slots
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity), "r"(0x989680u) : "memory");
     } while (!ok);
 }
 __device__ __forceinline__ void mbar_arrive(void *bar)
@@ -114,9 +115,9 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
     const float2 ri2 = __fmul2_rn(ri, ri);
     float2 k = __fmul2_rn(ri2, ri);
     if (SOFT) {
-        const float2 r = __fmul2_rn(r2, ri);
-        float2 t = __ffma2_rn(make_float2(c.C, c.C), r2, make_float2(c.A, c.A));
-        t = __ffma2_rn(make_float2(c.B, c.B), r, t);
+        const float2 r = __fmul2_rn(r2, ri);                // t = (C r + B) r + A: one register constant per FFMA2
+        float2 t = __ffma2_rn(r, make_float2(c.C, c.C), make_float2(c.B, c.B));
+        t = __ffma2_rn(t, r, make_float2(c.A, c.A));
         k.x = fminf(k.x, t.x);
         k.y = fminf(k.y, t.y);
     }
@@ -136,7 +137,7 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
     float k = ri * ri * ri;
     if (SOFT) {
         const float r = r2 * ri;
-        const float t = fmaf(c.B, r, fmaf(c.C, r2, c.A));
+        const float t = fmaf(fmaf(r, c.C, c.B), r, c.A);
         k = fminf(k, t);
     }
     ax = fmaf(k, dx, ax);
@@ -272,7 +273,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
                                 first = false;
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
-                                    d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy;
+                                    d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 8) | ((oy + 8) << 8);
                                     d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
@@ -343,6 +344,15 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
             const int np = d.npieces, soft_mode = d.soft_mode;
             const float sxi = d.dx - xi, syi = d.dy - yi;           // -(x_i - shift)
             const int ibase = zrel - d.j0;
+            // squared gap between the sink and the neighbour column (0 for the own column): a cell whose
+            // nearest face is farther than eps_s cannot hold a pair that needs the spline
+            float gxy2 = 0.f;
+            if (soft_mode == 1) {
+                const int ox = (d.oxy & 255) - 8, oy = (d.oxy >> 8) - 8;
+                const float gx = ox < 0 ? xi : (ox > 0 ? a.k.w_scaled - xi : 0.f);
+                const float gy = oy < 0 ? yi : (oy > 0 ? a.k.w_scaled - yi : 0.f);
+                gxy2 = fmaf(gx, gx, gy * gy);
+            }
             const float4 *sbase = reinterpret_cast<const float4 *>(&sm.buf[stage][0][0]);
             Partial f;
             f.clear();
@@ -361,7 +371,11 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                 const float szi = (float)(czs - oczs) - zi;
                 const float4 *px = sbase + (sm_off >> 2);
                 const int dt = t - R;
-                const bool soft = soft_mode == 2 || (soft_mode == 1 && dt >= -1 && dt <= 1);
+                bool soft = soft_mode == 2;
+                if (soft_mode == 1 && dt >= -1 && dt <= 1) {
+                    const float gz = dt < 0 ? zi : (dt > 0 ? a.k.w_scaled - zi : 0.f);
+                    soft = __any_sync(kFull, fmaf(gz, gz, gxy2) < a.k.soft_thr2);
+                }
                 if (soft) piece_loop<PACKED, true>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
                 else      piece_loop<PACKED, false>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
             }

@@ -70,6 +70,8 @@ struct Consts {          // everything the kernels need about the problem, by va
     float tiny;
     int fast_ok;                    // eps_s <= 0.999 cell_w: cells with max-norm offset >= 2 are pure Newtonian
     double out_scale;               // scale^2
+    float w_scaled;                 // cell width in scaled units, in [1,2)
+    float soft_thr2;                // (eps_s + rounding margin)^2 in scaled units: closer faces need the spline body
 };
 
 }  // namespace nf

@@ -130,6 +130,28 @@ def test_one_heavy_cell(oracle_mod):
     full_check(oracle_mod, pos, 6, 1.0, 2e-3, 2, what="one heavy cell")
 
 
+@pytest.mark.parametrize("cpd,eps", [(8, 0.004), (11, 0.002), (5, 0.03)])
+def test_close_pairs_across_faces(oracle_mod, cpd, eps):
+    """Pairs closer than eps_s that straddle cell faces, edges and corners (periodic ones included): the
+    kernel may take the Newtonian body only for cells whose nearest face is farther than eps_s.
+    Separations stay above 0.3 eps_s: the sink shift of a cross-face pair is rounded to 2^-24 cell widths
+    (tolerance), which is 1e-5 of a separation of 0.006 cell widths."""
+    rng = np.random.default_rng(cpd)
+    m = 3000
+    eps_s = 2.16 * eps
+    base = rng.integers(0, cpd, (m, 3)).astype(np.float64) / cpd          # a cell corner
+    free = rng.random((m, 3)) < 0.4                                         # axes along which the point is interior
+    p = base + np.where(free, rng.random((m, 3)) / cpd, 0.0)                # on a face / edge / corner
+    d = rng.normal(size=(m, 3))
+    d *= (rng.random((m, 1)) * 0.65 + 0.3) * eps_s / np.linalg.norm(d, axis=1, keepdims=True)
+    pos = np.concatenate([p - 0.5 * d, p + 0.5 * d, rng.random((2000, 3))]) % 1.0
+    pos = pos.astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    for fast in (1, 0):
+        full_check(oracle_mod, torch.from_numpy(pos), cpd, 1.0, eps, 2, options={"fastpath": fast},
+                   what=f"close pairs across faces cpd{cpd} fast{fast}")
+
+
 def test_coincident_particles(oracle_mod):
     g = torch.Generator().manual_seed(4)
     pos = torch.rand((500, 3), generator=g)

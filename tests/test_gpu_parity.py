@@ -85,6 +85,40 @@ def test_config4_full_size_sampled(oracle_mod):
     sampled_check(oracle_mod, nf_inputs.config(4), device="cuda")
 
 
+def test_config5_full_size_sampled(oracle_mod):
+    """Production-size config (1024^3 particles, ~26 GB of positions + accelerations): binning bit-exact at
+    full N, accelerations on the sink sample.  Needs ~60 GB of host memory for the oracle's arrays."""
+    import psutil
+    if psutil.virtual_memory().available < 70 * 2 ** 30:
+        pytest.skip("needs 70 GB of free host memory")
+    if torch.cuda.mem_get_info()[0] < 120 * 2 ** 30:
+        pytest.skip("needs 120 GB of free device memory")
+    cfg = nf_inputs.config(5)
+    import paper_2110_11398_b200 as nf
+    pos_dev = nf_inputs.generate(cfg, device="cuda")
+    torch.cuda.empty_cache()
+    pos = pos_dev.cpu().numpy()
+    b = oracle_mod.bin_particles(pos, cfg.cpd, cfg.L)
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos_dev)
+        acc = plan.accel()
+        torch.cuda.synchronize()
+        stats = plan.stats()
+        for k, v in plan.binning().items():            # one array at a time: 4.3 GB each
+            assert u32(v).tobytes() == b[k].tobytes(), f"binning array {k!r} differs from the oracle"
+            del v
+    del pos_dev
+    assert stats["interactions"] == oracle_mod.interactions(b["count"], cfg.cpd, cfg.R)
+    rng = np.random.default_rng(cfg.seed)
+    sinks = sample_sinks(b["count"], b["offset"], b["perm"], cfg.cpd, rng)
+    ref = oracle_mod.accel(pos, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=sinks, binning=b)
+    a_s = acc[torch.from_numpy(sinks).cuda()].cpu().numpy().astype(np.float64)
+    st = assert_parity(a_s, ref, cfg.name + " (sampled)")
+    tot = acc.double().sum(0).abs().max().item() / acc.double().abs().sum().item()
+    assert tot <= 2e-6
+    print(cfg.name, "sampled sinks", len(sinks), st, stats)
+
+
 # ---------------------------------------------------------------- closed forms through the GPU
 def test_golden_two_body_gpu():
     rows = [l.split() for l in open(os.path.join(GOLDEN, "two_body.txt")) if l.strip() and l[0] != "#"]

@@ -169,6 +169,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
         const double margin = 4.0 * 1.2e-7 * L * k.scale;
         const double thr = es + margin;
         k.soft_thr2 = (float)(thr * thr * 1.0001);
+        k.soft_r2 = (float)(es * es * 1.001 + 1e-30);     // eps = 0: only r = 0 (r^2 = tiny) is below it
     }
     p->eps = eps;
     p->device = -1;

@@ -53,7 +53,7 @@ struct __align__(16) StageDesc {
 };
 
 struct __align__(128) SharedStorage {
-    float buf[kStages][3][kTile];      // x, y, z of the staged sources
+    float buf[kStages][3][kTile + 4];  // x, y, z of the staged sources + one quad of dummies (never overwritten)
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
@@ -97,7 +97,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
-struct SoftCoef { float A, B, C, tiny; };
+struct SoftCoef { float A, B, C, tiny, soft_r2; };
 
 // two sources (packed) against one sink: 14 (soft) / 11 (Newtonian) FP32-pipe instructions per pair of
 // interactions, plus 2 MUFU.RSQ and, soft only, 2 FMNMX.
@@ -151,14 +151,55 @@ struct Partial {
     __device__ __forceinline__ void clear() { x = y = z = make_float2(0.f, 0.f); }
 };
 
+constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
+
+// Newtonian part of two packed interactions: d, r^2, 1/r and k = r^-3
+__device__ __forceinline__ void pair_head(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
+                                          const float2 nz, const float tiny, float2 &dx, float2 &dy, float2 &dz, float2 &r2,
+                                          float2 &ri, float2 &k)
+{
+    dx = __fadd2_rn(X, nx); dy = __fadd2_rn(Y, ny); dz = __fadd2_rn(Z, nz);
+    r2 = __ffma2_rn(dz, dz, make_float2(tiny, tiny));
+    r2 = __ffma2_rn(dy, dy, r2);
+    r2 = __ffma2_rn(dx, dx, r2);
+    ri.x = rsqrt_approx(r2.x);
+    ri.y = rsqrt_approx(r2.y);
+    k = __fmul2_rn(__fmul2_rn(ri, ri), ri);
+}
+__device__ __forceinline__ void pair_spline(const float2 r2, const float2 ri, const SoftCoef &c, float2 &k)
+{
+    const float2 r = __fmul2_rn(r2, ri);                    // t = (C r + B) r + A: one register constant per FFMA2
+    float2 t = __ffma2_rn(r, make_float2(c.C, c.C), make_float2(c.B, c.B));
+    t = __ffma2_rn(t, r, make_float2(c.A, c.A));
+    k.x = fminf(k.x, t.x);
+    k.y = fminf(k.y, t.y);
+}
+
+// Four sources against the sink of every lane.  All 32 lanes must call it together (warp vote inside).
+// SOFT: the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s --
+// a fraction of a percent of the quads at production density; otherwise the body is the Newtonian one
+// plus three FMNMX, a vote and a branch.
 template <bool PACKED, bool SOFT>
 __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float sxi, const float syi,
                                      const float szi, const SoftCoef &c, Partial &f)
 {
-    if (PACKED) {
+    if (PACKED && !SOFT) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        interact2<SOFT>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
-        interact2<SOFT>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2<false>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2<false>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
+    } else if (PACKED) {
+        const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
+        float2 dxa, dya, dza, r2a, ria, ka, dxb, dyb, dzb, r2b, rib, kb;
+        pair_head(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c.tiny, dxa, dya, dza, r2a, ria, ka);
+        pair_head(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c.tiny, dxb, dyb, dzb, r2b, rib, kb);
+        const float m = fminf(fminf(r2a.x, r2a.y), fminf(r2b.x, r2b.y));
+        if (__any_sync(kFull, m < c.soft_r2)) {
+            pair_spline(r2a, ria, c, ka);
+            pair_spline(r2b, rib, c, kb);
+        }
+        f.x = __ffma2_rn(ka, dxa, f.x); f.y = __ffma2_rn(ka, dya, f.y); f.z = __ffma2_rn(ka, dza, f.z);
+        f.x = __ffma2_rn(kb, dxb, f.x); f.y = __ffma2_rn(kb, dyb, f.y); f.z = __ffma2_rn(kb, dzb, f.z);
     } else {
         interact1<SOFT>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x);
         interact1<SOFT>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y);
@@ -168,17 +209,26 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 }
 
 // One step of a warp: every lane runs over ITS piece (n4 quads at px); nmin / nmax are the warp's smallest and
-// largest n4, so the first loop is uniform and only the ragged tail is predicated per lane.
+// largest n4.  The first loop is uniform; in the ragged tail a lane that has run out of sources is predicated
+// off (Newtonian body) or reads the stage's dummy quad (coordinates 2^55, contributes exactly 0) so that the
+// warp stays converged for the vote of the spline body.
 template <bool PACKED, bool SOFT>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
-                                           const float sxi, const float syi, const float szi, const SoftCoef &c, Partial &f)
+                                           const int jdummy, const float sxi, const float syi, const float szi,
+                                           const SoftCoef &c, Partial &f)
 {
-    const float4 *__restrict__ py = px + kTile / 4;
-    const float4 *__restrict__ pz = py + kTile / 4;
+    const float4 *__restrict__ py = px + kTileAlloc / 4;
+    const float4 *__restrict__ pz = py + kTileAlloc / 4;
 #pragma unroll 2
     for (int j = 0; j < nmin; j++) quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
-    for (int j = nmin; j < nmax; j++)
-        if (j < n4) quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+    for (int j = nmin; j < nmax; j++) {
+        if (SOFT && PACKED) {                         // the body votes: keep the warp converged
+            const int jj = j < n4 ? j : jdummy;
+            quad<PACKED, SOFT>(px[jj], py[jj], pz[jj], sxi, syi, szi, c, f);
+        } else if (j < n4) {
+            quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+        }
+    }
 }
 
 // ---- the kernel --------------------------------------------------------------------------------
@@ -192,8 +242,6 @@ struct AccelArgs {
     float *acc;                      // [n][3] input order
     int fastpath;
 };
-
-constexpr uint32_t kFull = 0xffffffffu;
 
 // The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
 // descriptors, the barriers and the TMA unit.
@@ -306,7 +354,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
 template <bool PACKED>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
 {
-    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny};
+    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2};
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;
@@ -370,14 +418,15 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                 const int nmin = __reduce_min_sync(kFull, n4);
                 const float szi = (float)(czs - oczs) - zi;
                 const float4 *px = sbase + (sm_off >> 2);
+                const int jdummy = (kTile - sm_off) >> 2;           // the dummy quad, relative to px
                 const int dt = t - R;
                 bool soft = soft_mode == 2;
                 if (soft_mode == 1 && dt >= -1 && dt <= 1) {
                     const float gz = dt < 0 ? zi : (dt > 0 ? a.k.w_scaled - zi : 0.f);
                     soft = __any_sync(kFull, fmaf(gz, gz, gxy2) < a.k.soft_thr2);
                 }
-                if (soft) piece_loop<PACKED, true>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
-                else      piece_loop<PACKED, false>(px, n4, nmin, nmax, sxi, syi, szi, coef, f);
+                if (soft) piece_loop<PACKED, true>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
+                else      piece_loop<PACKED, false>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
             }
             ax += (double)f.x.x + (double)f.x.y;
             ay += (double)f.y.x + (double)f.y.y;
@@ -401,6 +450,7 @@ __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(co
 {
     __shared__ SharedStorage sm;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid < kStages * 3 * 4) sm.buf[tid / 12][(tid / 4) % 3][kTile + (tid & 3)] = kDummy;
     if (tid == 0) {
         for (int s = 0; s < kStages; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kConsumerWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

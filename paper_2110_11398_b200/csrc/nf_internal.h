@@ -13,16 +13,16 @@ namespace nf {
 // ---- compile-time shape of the direct-sum kernel -------------------------------------------
 constexpr int kMaxR          = 4;                 // stencil (2R+1)^3 with R <= 4
 #ifndef NF_CONSUMER_WARPS
-#define NF_CONSUMER_WARPS 4
+#define NF_CONSUMER_WARPS 8
 #endif
 #ifndef NF_TILE
-#define NF_TILE 768
+#define NF_TILE 1024
 #endif
 #ifndef NF_STAGES
 #define NF_STAGES 3
 #endif
 #ifndef NF_MIN_CTAS
-#define NF_MIN_CTAS 6
+#define NF_MIN_CTAS 3
 #endif
 constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // sink lanes per CTA = 32 * kConsumerWarps
 constexpr int kChunk         = 32 * kConsumerWarps;   // max sinks per work unit (a window of one z-column)
@@ -71,6 +71,7 @@ struct Consts {          // everything the kernels need about the problem, by va
     int fast_ok;                    // eps_s <= 0.999 cell_w: cells with max-norm offset >= 2 are pure Newtonian
     double out_scale;               // scale^2
     float w_scaled;                 // cell width in scaled units, in [1,2)
+    float soft_r2;                  // eps_s^2 (scaled, with a 0.1 % margin): pairs below it take the spline
     float soft_thr2;                // (eps_s + rounding margin)^2 in scaled units: closer faces need the spline body
 };
 

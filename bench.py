@@ -24,6 +24,9 @@ if ROOT not in sys.path:
 METRIC = "near_field_pair_interactions_per_s"
 UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
+FLOPS_EXECUTED_MIN = 19         # the Newtonian body (3 add + 6 fma + 2 mul + rsqrt) the kernel runs where no pair is inside eps_s
+# DRAM bytes of one direct_kernel launch on config 3, ncu --set full (profiles/r1_v3_direct_kernel_config3.md)
+NCU_TRAFFIC_BYTES = {"config3_uniform_256": 960380928 + 656898304}
 L2_BYTES = 126 * 1024 * 1024
 
 
@@ -34,7 +37,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); default 3 = uniform 256^3")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--per-config", default="1,2,4", help="extra configs reported in 'per_config' (N=1 only); '' = none")
+    ap.add_argument("--per-config", default="1,2,4,5",
+                    help="extra configs reported in 'per_config' (N=1 only, 3 warm-ups + 3 steps; config 5: 1 + 1); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--fastpath", type=int, default=None)
@@ -302,7 +306,12 @@ def main_b200(args):
         "gpu_launches": K * (st["kernel_launches_bin"] + st["kernel_launches_accel"]),
         "clocks": r["clocks"],
         "roofline": {"bound": "alu", "kernel": "nf::direct_kernel<packed f32x2>", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                     "executed": {"flops_per_interaction": FLOPS_EXECUTED_MIN,
+                                  "achieved": achieved * FLOPS_EXECUTED_MIN / FLOPS_PER_INTERACTION,
+                                  "frac": achieved * FLOPS_EXECUTED_MIN / FLOPS_PER_INTERACTION / peak,
+                                  "note": "lower bound: quads with a pair inside eps_s execute the 25-flop body"},
+                     "attainable_frac": 0.88,
                      "peak_source": "SM count x 128 FP32 lanes x 2 x max SM clock read from the device (DESIGN.md)",
                      "sm_count": st["sm_count"], "clock_khz": st["clock_khz"], "launch_ms": ta * 1e3,
                      "grid": st["accel_grid"], "block": st["accel_block"]},
@@ -319,8 +328,9 @@ def main_b200(args):
         for idx in [int(t) for t in args.per_config.split(",") if t]:
             if idx == args.config:
                 continue
-            rr, _ = run_config(idx, args, local, None, with_e2e=False, steps=3, warmup=3)
-            per.append(summarise(rr))
+            big = idx == 5                                  # ~30 s per step: one warm-up, one timed step
+            rr, _ = run_config(idx, args, local, None, with_e2e=False, steps=1 if big else 3, warmup=1 if big else 3)
+            per.append(dict(summarise(rr), steps=rr["steps"], warmup=1 if big else 3))
         line["per_config"] = per
     print(json.dumps(line))
     if dist is not None:

@@ -22,8 +22,9 @@
 //   * coordinates are cell-corner relative (exact); the periodic wrap and the cell-to-cell shift are one
 //     constant per (sink cell, source cell) subtracted from the sink once per piece -- nothing periodic
 //     in the pair loop;
-//   * cells whose max-norm offset is >= 2 cannot hold a pair closer than eps_s (when eps_s <= cell width):
-//     they take the pure Newtonian body (no spline, no min);
+//   * the spline is evaluated only where it can matter: a source cell whose nearest face is farther than eps_s
+//     from every sink of the warp takes the pure Newtonian body; the others take min(r^2) over each quad of
+//     sources, vote, and evaluate (C r + B) r + A and the min only when some lane has a pair inside eps_s;
 //   * FP32 FMA chain per (sink, stage), stage partials added in FP64 (two-level accumulation);
 //   * the epilogue writes acc[perm[s]] directly (S7 fused, no sorted acceleration buffer).
 #include "nf_internal.h"
@@ -99,8 +100,9 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 // ---- pair bodies -------------------------------------------------------------------------------
 struct SoftCoef { float A, B, C, tiny, soft_r2; };
 
-// two sources (packed) against one sink: 14 (soft) / 11 (Newtonian) FP32-pipe instructions per pair of
-// interactions, plus 2 MUFU.RSQ and, soft only, 2 FMNMX.
+// two sources (packed) against one sink: 14 (spline) / 11 (Newtonian) FP32-pipe instructions per pair of
+// interactions, plus 2 MUFU.RSQ and, spline only, 2 FMNMX.  The kernel uses the Newtonian instance; the
+// spline of the packed path is pair_head / pair_spline below.
 template <bool SOFT>
 __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
                                           const float2 nz, const SoftCoef &c, float2 &ax, float2 &ay, float2 &az)

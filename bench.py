@@ -202,6 +202,21 @@ def time_e2e_steps(plan, pos_host, acc_host, steps, warmup):
     return (time.perf_counter() - t0) * 1e3
 
 
+def max_over_ranks(values, dist=None, device="cpu"):
+    """Replicas only: the ranks share no data; the one collective of the harness is the MAX of the timings."""
+    import torch
+    if dist is None:
+        return list(values)
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def aggregate_value(world, interactions, steps, total_ms):
+    """Whole-job interactions/s of `world` independent replicas that each ran `steps` steps in `total_ms` (max over ranks)."""
+    return world * interactions * steps / (total_ms / 1e3)
+
+
 def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, warmup=None):
     import torch
     import nf_inputs
@@ -276,17 +291,14 @@ def main_b200(args):
     st = r["stats"]
     t_total = r["total_ms"]
     e2e_ms = r["e2e_ms"]
-    if dist is not None:                       # max over ranks: replicas only, no data-path collective
-        tt = torch.tensor([t_total, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_total, e2e_ms = tt.tolist()
+    t_total, e2e_ms = max_over_ranks([t_total, e2e_ms], dist, "cuda")   # replicas only, no data-path collective
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
     s = summarise(r)
     I, n, K = r["interactions"], r["n"], r["steps"]
-    value = world * I * K / (t_total / 1e3)
+    value = aggregate_value(world, I, K, t_total)
     ta = statistics.mean(r["accel_ms"]) / 1e3
     peak = fp32_peak_tflops(st)
     achieved = FLOPS_PER_INTERACTION * I / ta / 1e12

@@ -10,6 +10,7 @@ from .nf_oracle import (  # noqa: F401
     kernel,
     bin_particles,
     accel,
+    density,
     interactions,
     num_threads,
     OracleError,

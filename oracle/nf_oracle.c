@@ -180,6 +180,58 @@ int nfo_accel(const float *pos, int64_t n, int cpd, double L, double eps, int R,
 }
 
 /*
+ * Kernel density estimate, computed by the paper "as part of the near-field force computation":
+ * "a kernel density estimate around all particles, using a weighting of 1 - r^2/b^2, where b is chosen
+ * to be 40% of the interparticle spacing" (sec. 3.3).
+ *   rho_i = sum_j max(0, 1 - r_ij^2 / b^2),  j over the particles of the (2R+1)^3 stencil cells of i,
+ * periodic image implied by the cell offset (reading C7).  Readings:
+ *   D1  the particle itself is part of the sum (weight 1 at r = 0), as is any coincident particle;
+ *   D2  b must not exceed R cell widths, so that the stencil holds every particle within b and the sum is
+ *       the plain periodic estimate (b = 0.4 spacings is 0.1 cell widths at the paper's 67 per cell).
+ *   sinks/m as in nfo_accel; rho [m] float64 out.
+ */
+int nfo_density(const float *pos, int64_t n, int cpd, double L, double b, int R,
+                const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
+                const int64_t *sinks, int64_t m, double *rho)
+{
+    if (nfo_check_args(cpd, L, 0.0, R) != NFO_OK || n < 0 || m < 0 || !(b > 0.0)) return NFO_ERR_ARG;
+    if (b > R * (L / cpd)) return NFO_ERR_ARG;
+    if (!sinks && m != n) return NFO_ERR_ARG;
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(|:bad)
+    for (int64_t k = 0; k < m; k++) {
+        int64_t i = sinks ? sinks[k] : k;
+        if (i < 0 || i >= n) { bad |= 1; continue; }
+        uint32_t id = cid[i];
+        int cz = (int)(id % (uint32_t)cpd);
+        int cy = (int)((id / (uint32_t)cpd) % (uint32_t)cpd);
+        int cx = (int)(id / ((uint32_t)cpd * (uint32_t)cpd));
+        double xi = (double)pos[3 * i + 0], yi = (double)pos[3 * i + 1], zi = (double)pos[3 * i + 2];
+        double sum = 0.0;
+        for (int ox = -R; ox <= R; ox++)
+        for (int oy = -R; oy <= R; oy++)
+        for (int oz = -R; oz <= R; oz++) {
+            int sx = cx + ox, sy = cy + oy, sz = cz + oz;
+            double wx = 0.0, wy = 0.0, wz = 0.0;
+            if (sx < 0) { sx += cpd; wx = -1.0; } else if (sx >= cpd) { sx -= cpd; wx = 1.0; }
+            if (sy < 0) { sy += cpd; wy = -1.0; } else if (sy >= cpd) { sy -= cpd; wy = 1.0; }
+            if (sz < 0) { sz += cpd; wz = -1.0; } else if (sz >= cpd) { sz -= cpd; wz = 1.0; }
+            int64_t c2 = ((int64_t)sx * cpd + sy) * cpd + sz;
+            for (uint32_t t = offset[c2]; t < offset[c2 + 1]; t++) {
+                int64_t j = perm[t];
+                double dx = (double)pos[3 * j + 0] - xi + wx * L;
+                double dy = (double)pos[3 * j + 1] - yi + wy * L;
+                double dz = (double)pos[3 * j + 2] - zi + wz * L;
+                double w = 1.0 - (dx * dx + dy * dy + dz * dz) / (b * b);
+                if (w > 0.0) sum += w;
+            }
+        }
+        rho[k] = sum;
+    }
+    return bad ? NFO_ERR_ARG : NFO_OK;
+}
+
+/*
  * Exact number of ordered pair evaluations of the definition (self pairs included):
  * I = sum_c count[c] * sum_{c' in stencil(c)} count[c'].
  */

@@ -44,6 +44,8 @@ def _load():
         lib.nfo_bin.argtypes = [vp, i64, i32, f64, vp, vp, vp, vp]
         lib.nfo_accel.restype = i32
         lib.nfo_accel.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
+        lib.nfo_density.restype = i32
+        lib.nfo_density.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_interactions.restype = i64
         lib.nfo_interactions.argtypes = [vp, i32, i32]
         _lib = lib
@@ -104,6 +106,25 @@ def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=N
                            binning["perm"].ctypes.data, sp, m, acc.ctypes.data)
     _check(rc, "nfo_accel")
     return acc
+
+
+def density(pos, cpd: int, L: float, b: float, R: int = 2, sinks=None, binning=None) -> np.ndarray:
+    """float64 kernel density estimate [m]: sum over the stencil of max(0, 1 - r^2/b^2), self included."""
+    pos = _pos32(pos)
+    n = pos.shape[0]
+    if binning is None:
+        binning = bin_particles(pos, cpd, L)
+    if sinks is None:
+        sp, m = None, n
+    else:
+        sinks = np.ascontiguousarray(sinks, dtype=np.int64)
+        sp, m = sinks.ctypes.data, sinks.shape[0]
+    rho = np.zeros(m, np.float64)
+    rc = _load().nfo_density(pos.ctypes.data, n, cpd, float(L), float(b), int(R),
+                             binning["cid"].ctypes.data, binning["offset"].ctypes.data,
+                             binning["perm"].ctypes.data, sp, m, rho.ctypes.data)
+    _check(rc, "nfo_density")
+    return rho
 
 
 def interactions(count, cpd: int, R: int = 2) -> int:

@@ -352,3 +352,70 @@ def test_interaction_count(oracle_mod):
                 for oz in range(-R, R + 1):
                     box += np.roll(c, (ox, oy, oz), axis=(0, 1, 2))
         assert oracle_mod.interactions(b["count"], cpd, R) == int((c * box).sum())
+
+
+# ---------------------------------------------------------------- kernel density estimate
+def _density_brute(pos, L, b):
+    """All pairs, particle-wise minimum image, NO cell mask: for b <= R cell widths the stencil holds every
+    particle within b, so the stencil sum is the plain periodic estimate (independent route, numpy)."""
+    p = pos.astype(np.float64)
+    d = p[None, :, :] - p[:, None, :]
+    d -= L * np.round(d / L)
+    r2 = (d ** 2).sum(-1)
+    return np.clip(1.0 - r2 / (b * b), 0.0, None).sum(1)
+
+
+def test_density_golden_two_body(oracle_mod):
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "density_two_body.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) >= 6
+    for row in rows:
+        cpd, R, b = int(row[0]), int(row[1]), float(row[2])
+        v = [float(t) for t in row[3:]]
+        pos = np.array([v[0:3], v[3:6]], np.float32)
+        rho = oracle_mod.density(pos, cpd, 1.0, b, R)
+        assert rho[0] == v[6] and rho[1] == v[6], (row, rho)
+
+
+@pytest.mark.parametrize("cpd,R,n,b", [(6, 2, 500, 0.05), (7, 2, 800, 2.0 / 7), (4, 1, 300, 0.2), (9, 3, 600, 0.11)])
+def test_density_brute_force(oracle_mod, cpd, R, n, b):
+    rng = np.random.default_rng(cpd * 100 + n)
+    pos = rng.random((n, 3), dtype=np.float32)
+    rho = oracle_mod.density(pos, cpd, 1.0, b, R)
+    np.testing.assert_allclose(rho, _density_brute(pos, 1.0, b), rtol=1e-12, atol=1e-12)
+
+
+def test_density_lattice_and_mean(oracle_mod):
+    """One particle per cell centre, b below the spacing: only the self term.  Uniform random particles: the mean
+    of rho - 1 is n_bar * integral of (1 - r^2/b^2) over the ball = n_bar * 8 pi b^3 / 15."""
+    cpd = 8
+    g = (np.stack(np.meshgrid(*[np.arange(cpd)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / cpd
+    assert np.all(oracle_mod.density(g.astype(np.float32), cpd, 1.0, 0.12, 2) == 1.0)
+    n, b = 200000, 0.03
+    pos = np.random.default_rng(5).random((n, 3), dtype=np.float32)
+    rho = oracle_mod.density(pos, 10, 1.0, b, 2)
+    expect = n * 8 * np.pi * b ** 3 / 15
+    sigma = np.sqrt(n * 4 * np.pi * b ** 3 * (1 / 3 - 2 / 5 + 1 / 7) / n)     # std of the mean over n sinks
+    assert abs((rho - 1).mean() - expect) < 6 * sigma, ((rho - 1).mean(), expect, sigma)
+
+
+def test_density_invariants(oracle_mod):
+    rng = np.random.default_rng(11)
+    pos = rng.random((3000, 3), dtype=np.float32)
+    b = 0.04
+    rho = oracle_mod.density(pos, 8, 1.0, b, 2)
+    assert rho.min() >= 1.0                                                 # the self term
+    # pair symmetry: sum_i (rho_i - 1) counts every pair twice with the same weight
+    d = pos[None].astype(np.float64) - pos[:, None].astype(np.float64)
+    d -= np.round(d)
+    w = np.clip(1 - (d ** 2).sum(-1) / b ** 2, 0, None)
+    assert abs((rho - 1).sum() - 2 * np.triu(w, 1).sum()) < 1e-9
+    # power-of-two scaling of (pos, L, b) leaves rho unchanged, exactly
+    assert np.array_equal(oracle_mod.density(pos * 4, 8, 4.0, b * 4, 2), rho)
+    # shuffle invariance and sink subsets
+    perm = rng.permutation(len(pos))
+    np.testing.assert_allclose(oracle_mod.density(pos[perm], 8, 1.0, b, 2), rho[perm], rtol=1e-13)
+    sinks = np.array([5, 17, 2999, 0])
+    assert np.array_equal(oracle_mod.density(pos, 8, 1.0, b, 2, sinks=sinks), rho[sinks])
+    # b larger than R cell widths would truncate the sum: rejected (reading D2)
+    with pytest.raises(oracle_mod.OracleError):
+        oracle_mod.density(pos, 8, 1.0, 0.26, 2)

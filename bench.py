@@ -40,6 +40,7 @@ def parse_args():
     ap.add_argument("--per-config", default="1,2,4,5",
                     help="extra configs reported in 'per_config' (N=1 only, 3 warm-ups + 3 steps; config 5: 1 + 1); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-density", action="store_true", help="skip the fused-density timing")
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--fastpath", type=int, default=None)
     ap.add_argument("--heavy-first", type=int, default=None)
@@ -244,6 +245,22 @@ def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, wa
                    l2="flushed between iterations (256 MiB write)" if flush is not None else "inputs exceed L2")
         a = acc.double()
         out["sum_check"] = float((a.sum(0).abs().max() / a.abs().sum()).item())   # total force ~ 0 at any size
+        if with_e2e and not args.no_density:
+            # the same pass with the fused kernel density estimate (b = 0.4 spacings)
+            rho = torch.empty(pos.shape[0], dtype=torch.float32, device="cuda")
+            b = 0.4 * cfg.L / cfg.n_side
+            evd = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            for _ in range(2):
+                plan.accel_density(b, acc, rho)
+            torch.cuda.synchronize()
+            evd[0].record()
+            for _ in range(steps):
+                plan.accel_density(b, acc, rho)
+            evd[1].record()
+            torch.cuda.synchronize()
+            out["density_ms_accel"] = evd[0].elapsed_time(evd[1]) / steps
+            out["density_mean"] = float(rho.double().mean().item())
+            del rho
         if with_e2e:
             pos_h = torch.empty(pos.shape, dtype=pos.dtype, pin_memory=True)
             pos_h.copy_(pos)
@@ -329,6 +346,11 @@ def main_b200(args):
                      "grid": st["accel_grid"], "block": st["accel_block"]},
         "sum_check": r["sum_check"],
     }
+    if "density_ms_accel" in r:
+        line["fused_density"] = {"call": "nf_accel_density, b = 0.4 interparticle spacings (PAPER.md:387)",
+                                 "ms_accel": r["density_ms_accel"], "ms_accel_forces_only": ta * 1e3,
+                                 "overhead_frac": r["density_ms_accel"] / (ta * 1e3) - 1.0,
+                                 "interactions_per_s": I / (r["density_ms_accel"] / 1e3), "mean_rho": r["density_mean"]}
     if r["clocks"].get("sm_mhz"):
         line["roofline"]["frac_at_sampled_clock"] = achieved / (peak * r["clocks"]["sm_mhz"] * 1e3 / st["clock_khz"])
     if not args.no_cpu_baseline and world == 1:

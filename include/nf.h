@@ -95,6 +95,19 @@ int nf_bin(nf_plan *plan, const float *pos_dev, long long n);
  */
 int nf_accel(nf_plan *plan, float *acc_dev);
 
+/*
+ * nf_accel_density -- nf_accel plus the kernel density estimate the paper computes "as part of the near-field
+ * force computation with minimal computational burden" (sec. 3.3), in the same pass:
+ *   rho_i = sum_j max(0, 1 - r_ij^2 / b^2),   j over the same (2R+1)^3 stencil particles, the particle itself
+ *   included (weight 1; reading D1).  The paper takes b = 0.4 interparticle spacings.
+ *   acc_dev  [n][3] float32, as nf_accel
+ *   rho_dev  [n] float32, device memory, OVERWRITTEN, row i = input particle i
+ *   b        kernel radius in box units, 0 < b <= R cell widths (then the stencil holds every particle
+ *            within b and the sum is the plain periodic estimate; reading D2), else NF_ERR_ARG
+ * Asynchronous like nf_accel.  Errors: NF_ERR_STATE, NF_ERR_ARG, NF_ERR_CUDA.
+ */
+int nf_accel_density(nf_plan *plan, float *acc_dev, float *rho_dev, double b);
+
 /* nf_destroy -- frees everything the plan allocated (never a caller workspace).  NULL-safe. */
 void nf_destroy(nf_plan *plan);
 

@@ -21,7 +21,7 @@ NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -
 _ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
 
 EXPORTS = [
-    "nf_plan_create", "nf_bin", "nf_accel", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
 ]
@@ -62,6 +62,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_bin.argtypes = [vp, vp, ll]
     lib.nf_accel.restype = i32
     lib.nf_accel.argtypes = [vp, vp]
+    lib.nf_accel_density.restype = i32
+    lib.nf_accel_density.argtypes = [vp, vp, vp, dbl]
     lib.nf_destroy.restype = None
     lib.nf_destroy.argtypes = [vp]
     lib.nf_bin_host.restype = i32
@@ -138,6 +140,14 @@ def nf_bin(plan: int, pos: torch.Tensor) -> None:
 def nf_accel(plan: int, acc: torch.Tensor) -> None:
     acc = _dev_f32(acc, "acc")
     _check(_lib.nf_accel(plan, ctypes.c_void_p(acc.data_ptr())))
+
+
+def nf_accel_density(plan: int, acc: torch.Tensor, rho: torch.Tensor, b: float) -> None:
+    acc = _dev_f32(acc, "acc")
+    if not (isinstance(rho, torch.Tensor) and rho.is_cuda and rho.dtype == torch.float32 and rho.is_contiguous()
+            and rho.dim() == 1 and rho.shape[0] == acc.shape[0]):
+        raise TypeError("rho must be a contiguous CUDA float32 tensor of shape [n]")
+    _check(_lib.nf_accel_density(plan, ctypes.c_void_p(acc.data_ptr()), ctypes.c_void_p(rho.data_ptr()), float(b)))
 
 
 def nf_bin_host(plan: int, pos_host: torch.Tensor) -> None:
@@ -247,6 +257,16 @@ class Plan:
             out = torch.empty((self.n, 3), dtype=torch.float32, device="cuda")
         nf_accel(self._h, out)
         return out
+
+    def accel_density(self, b: float, out: torch.Tensor | None = None, rho: torch.Tensor | None = None):
+        """Accelerations and the kernel density estimate of radius ``b`` in one pass; returns (acc, rho)."""
+        self._use_current_stream()
+        if out is None:
+            out = torch.empty((self.n, 3), dtype=torch.float32, device="cuda")
+        if rho is None:
+            rho = torch.empty((self.n,), dtype=torch.float32, device="cuda")
+        nf_accel_density(self._h, out, rho, b)
+        return out, rho
 
     def bin_host(self, pos_host: torch.Tensor):
         self._use_current_stream()

@@ -236,7 +236,21 @@ int nf_accel(nf_plan *p, float *acc)
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel called before a successful nf_bin"); return NF_ERR_STATE; }
     if (!acc && p->n > 0) { set_error("null acc"); return NF_ERR_ARG; }
-    return launch_accel(p, acc);
+    return launch_accel(p, acc, nullptr, 0.0);
+}
+
+int nf_accel_density(nf_plan *p, float *acc, float *rho, double b)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_accel_density called before a successful nf_bin"); return NF_ERR_STATE; }
+    if ((!acc || !rho) && p->n > 0) { set_error("null acc or rho"); return NF_ERR_ARG; }
+    if (!(b > 0.0) || !std::isfinite(b) || b > p->k.R * p->k.cell_w) {
+        set_error("density radius b = %g must be in (0, R cell widths = %g]: the stencil must hold every particle within b",
+                  b, p->k.R * p->k.cell_w);
+        return NF_ERR_ARG;
+    }
+    if (p->n == 0) return NF_OK;
+    return launch_accel(p, acc, rho, b);
 }
 
 int nf_bin_host(nf_plan *p, const float *pos_host, long long n)
@@ -259,7 +273,7 @@ int nf_accel_host(nf_plan *p, float *acc_host)
     if (!acc_host && p->n > 0) { set_error("null acc_host"); return NF_ERR_ARG; }
     int rc = ensure_stage(p, p->n);
     if (rc) return rc;
-    rc = launch_accel(p, p->acc_stage);
+    rc = launch_accel(p, p->acc_stage, nullptr, 0.0);
     if (rc) return rc;
     if (p->n > 0) NF_CUDA_OK(cudaMemcpyAsync(acc_host, p->acc_stage, (size_t)p->n * 12, cudaMemcpyDeviceToHost, p->stream));
     NF_CUDA_OK(cudaStreamSynchronize(p->stream));

@@ -98,7 +98,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
-struct SoftCoef { float A, B, C, tiny, soft_r2; };
+struct SoftCoef { float A, B, C, tiny, soft_r2, nb2; };   // nb2 = -1/b^2 of the density kernel
 
 // two sources (packed) against one sink: 14 (spline) / 11 (Newtonian) FP32-pipe instructions per pair of
 // interactions, plus 2 MUFU.RSQ and, spline only, 2 FMNMX.  The kernel uses the Newtonian instance; the
@@ -128,20 +128,22 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
     az = __ffma2_rn(k, dz, az);
 }
 
-// scalar body (variant 1): 14 / 11 FP32-pipe instructions per interaction
-template <bool SOFT>
+// scalar body (variant 1): 14 / 11 FP32-pipe instructions per interaction (+ 3 with the density estimate).
+// MODE 0: Newtonian, 1: spline, 2: spline + kernel density weight max(0, 1 - r^2/b^2)
+template <int MODE>
 __device__ __forceinline__ void interact1(const float X, const float Y, const float Z, const float nx, const float ny,
-                                          const float nz, const SoftCoef &c, float &ax, float &ay, float &az)
+                                          const float nz, const SoftCoef &c, float &ax, float &ay, float &az, float &rho)
 {
     const float dx = X + nx, dy = Y + ny, dz = Z + nz;
     const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, c.tiny)));
     const float ri = rsqrt_approx(r2);
     float k = ri * ri * ri;
-    if (SOFT) {
+    if (MODE >= 1) {
         const float r = r2 * ri;
         const float t = fmaf(fmaf(r, c.C, c.B), r, c.A);
         k = fminf(k, t);
     }
+    if (MODE == 2) rho += fmaxf(fmaf(r2, c.nb2, 1.0f), 0.0f);
     ax = fmaf(k, dx, ax);
     ay = fmaf(k, dy, ay);
     az = fmaf(k, dz, az);
@@ -149,8 +151,8 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
 
 // FP32 partial sums of one (sink, stage): two chains per component (packed: the two halves of an f32x2)
 struct Partial {
-    float2 x, y, z;
-    __device__ __forceinline__ void clear() { x = y = z = make_float2(0.f, 0.f); }
+    float2 x, y, z, rho;
+    __device__ __forceinline__ void clear() { x = y = z = rho = make_float2(0.f, 0.f); }
 };
 
 constexpr uint32_t kFull = 0xffffffffu;
@@ -177,16 +179,24 @@ __device__ __forceinline__ void pair_spline(const float2 r2, const float2 ri, co
     k.x = fminf(k.x, t.x);
     k.y = fminf(k.y, t.y);
 }
+// kernel density weights of two packed interactions: rho += max(0, 1 - r^2/b^2)
+__device__ __forceinline__ void pair_density(const float2 r2, const SoftCoef &c, float2 &rho)
+{
+    float2 w = __ffma2_rn(r2, make_float2(c.nb2, c.nb2), make_float2(1.0f, 1.0f));
+    w.x = fmaxf(w.x, 0.0f);
+    w.y = fmaxf(w.y, 0.0f);
+    rho = __fadd2_rn(rho, w);
+}
 
-// Four sources against the sink of every lane.  All 32 lanes must call it together (warp vote inside).
-// SOFT: the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s --
-// a fraction of a percent of the quads at production density; otherwise the body is the Newtonian one
-// plus three FMNMX, a vote and a branch.
-template <bool PACKED, bool SOFT>
+// Four sources against the sink of every lane.  With MODE >= 1 all 32 lanes must call it together (warp vote
+// inside): the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s -- a
+// fraction of a percent of the quads at production density; otherwise the body is the Newtonian one plus
+// three FMNMX, a vote and a branch.
+template <bool PACKED, int MODE>
 __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float sxi, const float syi,
                                      const float szi, const SoftCoef &c, Partial &f)
 {
-    if (PACKED && !SOFT) {
+    if (PACKED && MODE == 0) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
         interact2<false>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
         interact2<false>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
@@ -200,21 +210,25 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
             pair_spline(r2a, ria, c, ka);
             pair_spline(r2b, rib, c, kb);
         }
+        if (MODE == 2) {
+            pair_density(r2a, c, f.rho);
+            pair_density(r2b, c, f.rho);
+        }
         f.x = __ffma2_rn(ka, dxa, f.x); f.y = __ffma2_rn(ka, dya, f.y); f.z = __ffma2_rn(ka, dza, f.z);
         f.x = __ffma2_rn(kb, dxb, f.x); f.y = __ffma2_rn(kb, dyb, f.y); f.z = __ffma2_rn(kb, dzb, f.z);
     } else {
-        interact1<SOFT>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x);
-        interact1<SOFT>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y);
-        interact1<SOFT>(X.z, Y.z, Z.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x);
-        interact1<SOFT>(X.w, Y.w, Z.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y);
+        interact1<MODE>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
+        interact1<MODE>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
+        interact1<MODE>(X.z, Y.z, Z.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
+        interact1<MODE>(X.w, Y.w, Z.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
     }
 }
 
 // One step of a warp: every lane runs over ITS piece (n4 quads at px); nmin / nmax are the warp's smallest and
 // largest n4.  The first loop is uniform; in the ragged tail a lane that has run out of sources is predicated
-// off (Newtonian body) or reads the stage's dummy quad (coordinates 2^55, contributes exactly 0) so that the
-// warp stays converged for the vote of the spline body.
-template <bool PACKED, bool SOFT>
+// off (Newtonian body) or reads the stage's dummy quad (coordinates 2^55: contributes exactly 0 to the force
+// and to the density) so that the warp stays converged for the vote of the spline body.
+template <bool PACKED, int MODE>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
                                            const int jdummy, const float sxi, const float syi, const float szi,
                                            const SoftCoef &c, Partial &f)
@@ -222,13 +236,13 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
     const float4 *__restrict__ py = px + kTileAlloc / 4;
     const float4 *__restrict__ pz = py + kTileAlloc / 4;
 #pragma unroll 2
-    for (int j = 0; j < nmin; j++) quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+    for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
     for (int j = nmin; j < nmax; j++) {
-        if (SOFT && PACKED) {                         // the body votes: keep the warp converged
+        if (MODE >= 1 && PACKED) {                    // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
-            quad<PACKED, SOFT>(px[jj], py[jj], pz[jj], sxi, syi, szi, c, f);
+            quad<PACKED, MODE>(px[jj], py[jj], pz[jj], sxi, syi, szi, c, f);
         } else if (j < n4) {
-            quad<PACKED, SOFT>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+            quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
         }
     }
 }
@@ -243,6 +257,11 @@ struct AccelArgs {
     uint32_t *counter;               // atomic work counter (zeroed before launch)
     float *acc;                      // [n][3] input order
     int fastpath;
+    // kernel density estimate (DENS kernels only)
+    float *rho;                      // [n] input order
+    float dens_nb2;                  // -1 / b^2, scaled units
+    float dens_thr2;                 // (b + rounding margin)^2: closer faces can hold a pair inside b
+    int dens_mode;                   // 1: b < cell width, only touching cells whose face is within b; 2: every cell
 };
 
 // The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
@@ -353,15 +372,15 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED>
+template <bool PACKED, bool DENS>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
 {
-    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2};
+    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f};
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;
     float xi = 0.f, yi = 0.f, zi = 0.f;
-    double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0;
+    double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0, rho = 0.0;
     int zrel = 0;                       // the lane's sink cell, relative to z0
     uint32_t slot = 0;                  // the lane's sorted slot (perm index)
     bool act = false, warp_on = false;
@@ -374,7 +393,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
             const uint32_t ns = d.ns, kk = (uint32_t)(warp * 32 + lane);
             warp_on = (uint32_t)(warp * 32) < ns;
             act = kk < ns;
-            ax = ay = az = 0.0;
+            ax = ay = az = rho = 0.0;
             if (warp_on) {
                 // lanes past the end of a ragged window shadow its last sink (same pieces, nothing written)
                 slot = d.s0 + (act ? kk : ns - 1u);
@@ -397,8 +416,10 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
             // squared gap between the sink and the neighbour column (0 for the own column): a cell whose
             // nearest face is farther than eps_s cannot hold a pair that needs the spline
             float gxy2 = 0.f;
-            if (soft_mode == 1) {
-                const int ox = (d.oxy & 255) - 8, oy = (d.oxy >> 8) - 8;
+            const int ox = (d.oxy & 255) - 8, oy = (d.oxy >> 8) - 8;
+            const bool near_col = ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1;
+            const bool gap_dens = DENS && a.dens_mode == 1 && near_col;
+            if (soft_mode == 1 || gap_dens) {
                 const float gx = ox < 0 ? xi : (ox > 0 ? a.k.w_scaled - xi : 0.f);
                 const float gy = oy < 0 ? yi : (oy > 0 ? a.k.w_scaled - yi : 0.f);
                 gxy2 = fmaf(gx, gx, gy * gy);
@@ -422,17 +443,21 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                 const float4 *px = sbase + (sm_off >> 2);
                 const int jdummy = (kTile - sm_off) >> 2;           // the dummy quad, relative to px
                 const int dt = t - R;
-                bool soft = soft_mode == 2;
-                if (soft_mode == 1 && dt >= -1 && dt <= 1) {
+                bool soft = soft_mode == 2, dens = DENS && a.dens_mode == 2;
+                if ((soft_mode == 1 || gap_dens) && dt >= -1 && dt <= 1) {
                     const float gz = dt < 0 ? zi : (dt > 0 ? a.k.w_scaled - zi : 0.f);
-                    soft = __any_sync(kFull, fmaf(gz, gz, gxy2) < a.k.soft_thr2);
+                    const float gap2 = fmaf(gz, gz, gxy2);
+                    if (soft_mode == 1) soft = __any_sync(kFull, gap2 < a.k.soft_thr2);
+                    if (gap_dens) dens = __any_sync(kFull, gap2 < a.dens_thr2);
                 }
-                if (soft) piece_loop<PACKED, true>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
-                else      piece_loop<PACKED, false>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
+                if (DENS && dens) piece_loop<PACKED, 2>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
+                else if (soft)    piece_loop<PACKED, 1>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
+                else              piece_loop<PACKED, 0>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
             }
             ax += (double)f.x.x + (double)f.x.y;
             ay += (double)f.y.x + (double)f.y.y;
             az += (double)f.z.x + (double)f.z.y;
+            if (DENS) rho += (double)f.rho.x + (double)f.rho.y;
         }
         if ((flags & kFlagEnd) && act) {
             const size_t i = __ldg(a.perm + slot);
@@ -440,6 +465,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
             a.acc[3 * i + 0] = (float)(ax * s2);
             a.acc[3 * i + 1] = (float)(ay * s2);
             a.acc[3 * i + 2] = (float)(az * s2);
+            if (DENS) a.rho[i] = (float)rho;
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[stage]);
@@ -447,7 +473,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED>
+template <bool PACKED, bool DENS>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
     __shared__ SharedStorage sm;
@@ -459,26 +485,35 @@ __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(co
     }
     __syncthreads();
     if (warp == kConsumerWarps) producer(a, sm, lane);
-    else                        consumer<PACKED>(a, sm, warp, lane);
+    else                        consumer<PACKED, DENS>(a, sm, warp, lane);
+}
+
+typedef void (*direct_fn)(const AccelArgs);
+static direct_fn pick_kernel(int variant, bool dens)
+{
+    if (variant == 0) return dens ? direct_kernel<true, true> : direct_kernel<true, false>;
+    return dens ? direct_kernel<false, true> : direct_kernel<false, false>;
 }
 
 int accel_max_ctas_per_sm(int variant)
 {
     int nb = 0;
-    cudaError_t e = variant == 0
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, direct_kernel<true>, kAccelThreads, 0)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, direct_kernel<false>, kAccelThreads, 0);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick_kernel(variant, false), kAccelThreads, 0);
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
 
-int launch_accel(nf_plan *p, float *acc)
+// rho == NULL: forces only.  b is the density kernel radius in box units (validated by the caller).
+int launch_accel(nf_plan *p, float *acc, float *rho, double b)
 {
     cudaStream_t st = p->stream;
     p->have_accel_time = false;
     p->launches_accel = 0;
     if (p->n == 0 || p->n_units == 0) return NF_OK;
-    int per_sm = accel_max_ctas_per_sm(p->variant);
+    const bool dens = rho != nullptr;
+    direct_fn fn = pick_kernel(p->variant, dens);
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
     if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
     if (p->ctas_per_sm > 0 && p->ctas_per_sm < per_sm) per_sm = p->ctas_per_sm;
     long long grid = (long long)p->sm_count * per_sm;
@@ -492,10 +527,17 @@ int launch_accel(nf_plan *p, float *acc)
     a.counter = &p->ws.scalars[1];
     a.acc = acc;
     a.fastpath = p->fastpath;
+    a.rho = rho; a.dens_nb2 = 0.f; a.dens_thr2 = 0.f; a.dens_mode = 0;
+    if (dens) {
+        const double bs = b * p->k.scale;                       // scaled units
+        const double margin = 4.0 * 1.2e-7 * p->k.L * p->k.scale;   // as for the spline: float32 rounding of the coordinates
+        a.dens_nb2 = (float)(-1.0 / (bs * bs));
+        a.dens_thr2 = (float)((bs + margin) * (bs + margin) * 1.0001);
+        a.dens_mode = (b <= 0.999 * p->k.cell_w) ? 1 : 2;
+    }
     NF_CUDA_OK(cudaEventRecord(p->ev[2], st));
     NF_CUDA_OK(cudaMemsetAsync(a.counter, 0, 4, st));
-    if (p->variant == 0) direct_kernel<true><<<(unsigned)grid, kAccelThreads, 0, st>>>(a);
-    else                 direct_kernel<false><<<(unsigned)grid, kAccelThreads, 0, st>>>(a);
+    fn<<<(unsigned)grid, kAccelThreads, 0, st>>>(a);
     NF_CUDA_OK(cudaGetLastError());
     NF_CUDA_OK(cudaEventRecord(p->ev[3], st));
     p->have_accel_time = true;

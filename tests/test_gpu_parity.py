@@ -299,3 +299,90 @@ def test_errors_gpu():
                 p.accel(torch.empty((2, 3), device="cuda"))
         p.bin(torch.rand((10, 3), device="cuda"))      # the plan recovers
         p.accel()
+
+
+# ---------------------------------------------------------------- fused kernel density estimate
+TOL_RHO = 1e-5   # |rho_gpu - rho_ref| <= TOL_RHO * rho_ref for every particle (weights are O(1), rho >= 1)
+
+
+def density_check(oracle_mod, pos_cpu, cpd, L, eps, b, R=2, options=None, sinks=None, what=""):
+    import paper_2110_11398_b200 as nf
+    pos = pos_cpu.numpy()
+    with nf.Plan(cpd, L, eps, R) as plan:
+        for k, v in (options or {}).items():
+            plan.set_option(k, v)
+        plan.bin(pos_cpu.cuda())
+        acc, rho = plan.accel_density(b)
+        acc0 = plan.accel()
+        torch.cuda.synchronize()
+    bn = oracle_mod.bin_particles(pos, cpd, L)
+    ref_rho = oracle_mod.density(pos, cpd, L, b, R, sinks=sinks, binning=bn)
+    ref_acc = oracle_mod.accel(pos, cpd, L, eps, R, sinks=sinks, binning=bn)
+    g_rho = rho.cpu().numpy().astype(np.float64)
+    g_acc = acc.cpu().numpy().astype(np.float64)
+    if sinks is not None:
+        g_rho, g_acc = g_rho[sinks], g_acc[sinks]
+    err = np.abs(g_rho - ref_rho) / ref_rho
+    assert err.max() <= TOL_RHO, f"{what}: density rel. error {err.max():.3e}"
+    st = assert_parity(g_acc, ref_acc, what + " (accelerations of the fused pass)")
+    # the force-only pass and the fused pass agree to rounding
+    d = (acc - acc0).norm(dim=1) / acc0.norm(dim=1).clamp_min(1e-30)
+    assert d.max().item() <= 1e-5
+    return {"rho_max_err": float(err.max()), "rho_mean": float(ref_rho.mean()), **st}
+
+
+def test_density_golden_gpu():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "density_two_body.txt")) if l.strip() and l[0] != "#"]
+    import paper_2110_11398_b200 as nf
+    for row in rows:
+        cpd, R, b = int(row[0]), int(row[1]), float(row[2])
+        v = [float(t) for t in row[3:]]
+        pos = torch.tensor([v[0:3], v[3:6]], dtype=torch.float32)
+        with nf.Plan(cpd, 1.0, 1e-6, R) as p:
+            p.bin(pos.cuda())
+            _, rho = p.accel_density(b)
+        assert np.abs(rho.cpu().numpy() - v[6]).max() <= 1e-6, (row, rho)
+
+
+@pytest.mark.parametrize("idx,n_side,cpd", [(1, 32, 9), (2, 48, 12), (4, 40, 10), (5, 40, 10)])
+def test_density_scaled_configs(oracle_mod, idx, n_side, cpd):
+    """b = 0.4 interparticle spacings on the config recipes, every particle compared."""
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    st = density_check(oracle_mod, nf_inputs.generate(cfg), cfg.cpd, cfg.L, cfg.eps, 0.4 * cfg.L / cfg.n_side, cfg.R, what=cfg.name)
+    print(cfg.name, st)
+
+
+@pytest.mark.parametrize("cpd,R,bw,variant", [(6, 2, 1.5, 0), (6, 2, 2.0, 1), (5, 2, 0.3, 1), (7, 3, 0.999, 0), (3, 1, 1.0, 0),
+                                             (8, 2, 0.05, 0)])
+def test_density_radius_sweep(oracle_mod, cpd, R, bw, variant):
+    """b from a small fraction of a cell up to R cell widths (kernel reaching every stencil cell), both kernel variants."""
+    g = torch.Generator().manual_seed(cpd * 7 + R)
+    pos = torch.rand((5000, 3), generator=g)
+    st = density_check(oracle_mod, pos, cpd, 1.0, 0.004, bw / cpd, R, options={"variant": variant}, what=f"b={bw} cells")
+    print(st)
+
+
+def test_density_config3_full_size_sampled(oracle_mod):
+    cfg = nf_inputs.config(3)
+    pos = nf_inputs.generate(cfg)
+    bn = oracle_mod.bin_particles(pos.numpy(), cfg.cpd, cfg.L)
+    sinks = sample_sinks(bn["count"], bn["offset"], bn["perm"], cfg.cpd, np.random.default_rng(3), n_random=600)
+    st = density_check(oracle_mod, pos, cfg.cpd, cfg.L, cfg.eps, 0.4 * cfg.L / cfg.n_side, cfg.R, sinks=sinks, what=cfg.name)
+    print(cfg.name, "density, sampled sinks", len(sinks), st)
+
+
+def test_density_errors_and_empty():
+    import paper_2110_11398_b200 as nf
+    B = nf.binding
+    with nf.Plan(5, 1.0, 0.01, 2) as p:
+        with pytest.raises(nf.NFError) as e:
+            p.accel_density(0.05)
+        assert e.value.code == B.NF_ERR_STATE
+        p.bin(torch.rand((100, 3), device="cuda"))
+        for bad in (0.0, -1.0, 0.41, float("nan")):             # R cell widths = 0.4
+            with pytest.raises(nf.NFError) as e:
+                p.accel_density(bad)
+            assert e.value.code == B.NF_ERR_ARG
+        p.bin(torch.zeros((0, 3), device="cuda"))
+        a, r = p.accel_density(0.1)
+        assert a.shape == (0, 3) and r.shape == (0,)

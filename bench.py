@@ -261,6 +261,19 @@ def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, wa
             out["density_ms_accel"] = evd[0].elapsed_time(evd[1]) / steps
             out["density_mean"] = float(rho.double().mean().item())
             del rho
+            # kick and per-cell max |a| fused into the epilogue
+            vel = torch.zeros_like(pos)
+            amax = torch.empty(cfg.cpd ** 3, dtype=torch.float32, device="cuda")
+            nf.nf_accel_kick(plan._h, acc, vel, 1e-6, amax)
+            torch.cuda.synchronize()
+            evd[0].record()
+            for _ in range(steps):
+                nf.nf_accel_kick(plan._h, acc, vel, 1e-6, amax)
+            evd[1].record()
+            torch.cuda.synchronize()
+            out["kick_ms_accel"] = evd[0].elapsed_time(evd[1]) / steps
+            out["amax_global"] = float(amax.max().item())
+            del vel, amax
         if with_e2e:
             pos_h = torch.empty(pos.shape, dtype=pos.dtype, pin_memory=True)
             pos_h.copy_(pos)
@@ -351,6 +364,10 @@ def main_b200(args):
                                  "ms_accel": r["density_ms_accel"], "ms_accel_forces_only": ta * 1e3,
                                  "overhead_frac": r["density_ms_accel"] / (ta * 1e3) - 1.0,
                                  "interactions_per_s": I / (r["density_ms_accel"] / 1e3), "mean_rho": r["density_mean"]}
+    if "kick_ms_accel" in r:
+        line["fused_kick"] = {"call": "nf_accel_kick: v += a dt and per-cell max |a| in the epilogue (PAPER.md:353, 212)",
+                              "ms_accel": r["kick_ms_accel"], "overhead_frac": r["kick_ms_accel"] / (ta * 1e3) - 1.0,
+                              "max_accel": r["amax_global"]}
     if r["clocks"].get("sm_mhz"):
         line["roofline"]["frac_at_sampled_clock"] = achieved / (peak * r["clocks"]["sm_mhz"] * 1e3 / st["clock_khz"])
     if not args.no_cpu_baseline and world == 1:

@@ -108,6 +108,22 @@ int nf_accel(nf_plan *plan, float *acc_dev);
  */
 int nf_accel_density(nf_plan *plan, float *acc_dev, float *rho_dev, double b);
 
+/*
+ * nf_accel_kick -- nf_accel with the two steps that follow the near field in the paper's pipeline fused into
+ * the kernel epilogue (no second pass over the accelerations):
+ *   - the leapfrog kick  v_i += a_i * dt                      ("kicks the particle velocities")
+ *   - the per-cell maximum particle acceleration max_i |a_i|  (the denominator of the timestep criterion,
+ *     "the per-cell maximum particle acceleration")
+ *   acc_dev        [n][3] float32 or NULL (accelerations not stored)
+ *   vel_dev        [n][3] float32, input order, UPDATED IN PLACE with one float32 FMA per component, or NULL
+ *   dt             kick factor (finite)
+ *   amax_cell_dev  [cpd^3] float32, OVERWRITTEN: max over the particles of the cell of the Euclidean norm of the
+ *                  float32 acceleration, 0 for an empty cell; or NULL
+ * At least one of the three pointers must be non-NULL.  Asynchronous like nf_accel.
+ * Errors: NF_ERR_STATE, NF_ERR_ARG, NF_ERR_CUDA.
+ */
+int nf_accel_kick(nf_plan *plan, float *acc_dev, float *vel_dev, double dt, float *amax_cell_dev);
+
 /* nf_destroy -- frees everything the plan allocated (never a caller workspace).  NULL-safe. */
 void nf_destroy(nf_plan *plan);
 

@@ -11,6 +11,8 @@ from .nf_oracle import (  # noqa: F401
     bin_particles,
     accel,
     density,
+    kick,
+    cell_max_accel,
     interactions,
     num_threads,
     OracleError,

@@ -127,6 +127,20 @@ def density(pos, cpd: int, L: float, b: float, R: int = 2, sinks=None, binning=N
     return rho
 
 
+def kick(vel, acc, dt: float) -> np.ndarray:
+    """Leapfrog kick v + a dt in float64 ("kicks the particle velocities")."""
+    return np.asarray(vel, np.float64) + np.asarray(acc, np.float64) * float(dt)
+
+
+def cell_max_accel(acc, cid, ncells: int) -> np.ndarray:
+    """Per-cell maximum of the Euclidean norm of the particle accelerations, 0 for empty cells: "the per-cell
+    maximum particle acceleration" of the timestep criterion.  acc [n][3], cid [n] cell ids."""
+    norm = np.sqrt((np.asarray(acc, np.float64) ** 2).sum(axis=1))
+    out = np.zeros(int(ncells), np.float64)
+    np.maximum.at(out, np.asarray(cid, np.int64), norm)
+    return out
+
+
 def interactions(count, cpd: int, R: int = 2) -> int:
     """Exact ordered-pair count of the definition (self pairs included)."""
     count = np.ascontiguousarray(count, dtype=np.uint32)

@@ -21,7 +21,7 @@ NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -
 _ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
 
 EXPORTS = [
-    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
 ]
@@ -64,6 +64,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_accel.argtypes = [vp, vp]
     lib.nf_accel_density.restype = i32
     lib.nf_accel_density.argtypes = [vp, vp, vp, dbl]
+    lib.nf_accel_kick.restype = i32
+    lib.nf_accel_kick.argtypes = [vp, vp, vp, dbl, vp]
     lib.nf_destroy.restype = None
     lib.nf_destroy.argtypes = [vp]
     lib.nf_bin_host.restype = i32
@@ -148,6 +150,18 @@ def nf_accel_density(plan: int, acc: torch.Tensor, rho: torch.Tensor, b: float) 
             and rho.dim() == 1 and rho.shape[0] == acc.shape[0]):
         raise TypeError("rho must be a contiguous CUDA float32 tensor of shape [n]")
     _check(_lib.nf_accel_density(plan, ctypes.c_void_p(acc.data_ptr()), ctypes.c_void_p(rho.data_ptr()), float(b)))
+
+
+def nf_accel_kick(plan: int, acc: torch.Tensor | None, vel: torch.Tensor | None, dt: float,
+                  amax_cell: torch.Tensor | None) -> None:
+    pa = ctypes.c_void_p(_dev_f32(acc, "acc").data_ptr()) if acc is not None else None
+    pv = ctypes.c_void_p(_dev_f32(vel, "vel").data_ptr()) if vel is not None else None
+    pm = None
+    if amax_cell is not None:
+        if not (amax_cell.is_cuda and amax_cell.dtype == torch.float32 and amax_cell.is_contiguous() and amax_cell.dim() == 1):
+            raise TypeError("amax_cell must be a contiguous CUDA float32 tensor of shape [cpd^3]")
+        pm = ctypes.c_void_p(amax_cell.data_ptr())
+    _check(_lib.nf_accel_kick(plan, pa, pv, float(dt), pm))
 
 
 def nf_bin_host(plan: int, pos_host: torch.Tensor) -> None:
@@ -267,6 +281,18 @@ class Plan:
             rho = torch.empty((self.n,), dtype=torch.float32, device="cuda")
         nf_accel_density(self._h, out, rho, b)
         return out, rho
+
+    def accel_kick(self, vel: torch.Tensor | None, dt: float, out: torch.Tensor | None = None, want_amax: bool = True,
+                   store_acc: bool = True):
+        """Accelerations, kick of ``vel`` in place and per-cell max |a| in one pass; returns (acc, amax_cell)."""
+        self._use_current_stream()
+        if out is None and store_acc:
+            out = torch.empty((self.n, 3), dtype=torch.float32, device="cuda")
+        if vel is not None and vel.shape[0] != self.n:
+            raise ValueError("vel must have one row per binned particle")
+        amax = torch.empty((self.ncells,), dtype=torch.float32, device="cuda") if want_amax else None
+        nf_accel_kick(self._h, out if store_acc else None, vel, dt, amax)
+        return out, amax
 
     def bin_host(self, pos_host: torch.Tensor):
         self._use_current_stream()

@@ -236,7 +236,7 @@ int nf_accel(nf_plan *p, float *acc)
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel called before a successful nf_bin"); return NF_ERR_STATE; }
     if (!acc && p->n > 0) { set_error("null acc"); return NF_ERR_ARG; }
-    return launch_accel(p, acc, nullptr, 0.0);
+    return launch_accel(p, acc, nullptr, 0.0, nullptr, 0.0, nullptr);
 }
 
 int nf_accel_density(nf_plan *p, float *acc, float *rho, double b)
@@ -250,7 +250,20 @@ int nf_accel_density(nf_plan *p, float *acc, float *rho, double b)
         return NF_ERR_ARG;
     }
     if (p->n == 0) return NF_OK;
-    return launch_accel(p, acc, rho, b);
+    return launch_accel(p, acc, rho, b, nullptr, 0.0, nullptr);
+}
+
+int nf_accel_kick(nf_plan *p, float *acc, float *vel, double dt, float *amax_cell)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_accel_kick called before a successful nf_bin"); return NF_ERR_STATE; }
+    if (!acc && !vel && !amax_cell) { set_error("nf_accel_kick: acc, vel and amax_cell are all null"); return NF_ERR_ARG; }
+    if (!std::isfinite(dt)) { set_error("dt must be finite"); return NF_ERR_ARG; }
+    if (p->n == 0) {
+        if (amax_cell) NF_CUDA_OK(cudaMemsetAsync(amax_cell, 0, 4 * (size_t)p->k.ncells, p->stream));
+        return NF_OK;
+    }
+    return launch_accel(p, acc, nullptr, 0.0, vel, dt, amax_cell);
 }
 
 int nf_bin_host(nf_plan *p, const float *pos_host, long long n)
@@ -273,7 +286,7 @@ int nf_accel_host(nf_plan *p, float *acc_host)
     if (!acc_host && p->n > 0) { set_error("null acc_host"); return NF_ERR_ARG; }
     int rc = ensure_stage(p, p->n);
     if (rc) return rc;
-    rc = launch_accel(p, p->acc_stage, nullptr, 0.0);
+    rc = launch_accel(p, p->acc_stage, nullptr, 0.0, nullptr, 0.0, nullptr);
     if (rc) return rc;
     if (p->n > 0) NF_CUDA_OK(cudaMemcpyAsync(acc_host, p->acc_stage, (size_t)p->n * 12, cudaMemcpyDeviceToHost, p->stream));
     NF_CUDA_OK(cudaStreamSynchronize(p->stream));

@@ -262,6 +262,10 @@ struct AccelArgs {
     float dens_nb2;                  // -1 / b^2, scaled units
     float dens_thr2;                 // (b + rounding margin)^2: closer faces can hold a pair inside b
     int dens_mode;                   // 1: b < cell width, only touching cells whose face is within b; 2: every cell
+    // fused epilogue: leapfrog kick and per-cell maximum acceleration; any may be NULL
+    float *vel;                      // [n][3] input order, v += a * dt in float32
+    float dt;
+    uint32_t *amax;                  // [cpd^3] bit patterns of non-negative floats, zeroed before launch
 };
 
 // The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
@@ -372,7 +376,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED, bool DENS>
+template <bool PACKED, bool DENS, bool EPI>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
 {
     const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f};
@@ -383,6 +387,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
     double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0, rho = 0.0;
     int zrel = 0;                       // the lane's sink cell, relative to z0
     uint32_t slot = 0;                  // the lane's sorted slot (perm index)
+    uint32_t cell = 0;                  // the lane's sink cell id
     bool act = false, warp_on = false;
     for (;;) {
         mbar_wait(&sm.full[stage], phase);
@@ -404,6 +409,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                     if (__ldg(off + mid) <= slot) lo = mid; else hi = mid - 1;
                 }
                 zrel = lo - (int)d.z0;
+                if (EPI) cell = d.colbase + (uint32_t)lo;
                 const uint32_t p = __ldg(a.poff + d.colbase + lo) + (slot - __ldg(off + lo));
                 xi = __ldg(a.x + p); yi = __ldg(a.y + p); zi = __ldg(a.z + p);
                 oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
@@ -462,10 +468,16 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
         if ((flags & kFlagEnd) && act) {
             const size_t i = __ldg(a.perm + slot);
             const double s2 = a.k.out_scale;
-            a.acc[3 * i + 0] = (float)(ax * s2);
-            a.acc[3 * i + 1] = (float)(ay * s2);
-            a.acc[3 * i + 2] = (float)(az * s2);
+            const float fx = (float)(ax * s2), fy = (float)(ay * s2), fz = (float)(az * s2);
+            if (!EPI || a.acc) { a.acc[3 * i + 0] = fx; a.acc[3 * i + 1] = fy; a.acc[3 * i + 2] = fz; }
             if (DENS) a.rho[i] = (float)rho;
+            if (EPI && a.vel) {                                   // kick: v += a dt (leapfrog)
+                a.vel[3 * i + 0] = fmaf(fx, a.dt, a.vel[3 * i + 0]);
+                a.vel[3 * i + 1] = fmaf(fy, a.dt, a.vel[3 * i + 1]);
+                a.vel[3 * i + 2] = fmaf(fz, a.dt, a.vel[3 * i + 2]);
+            }
+            if (EPI && a.amax)                             // per-cell max |a| of the timestep criterion
+                atomicMax(a.amax + cell, __float_as_uint(sqrtf(fmaf(fx, fx, fmaf(fy, fy, fz * fz)))));
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[stage]);
@@ -473,7 +485,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED, bool DENS>
+template <bool PACKED, bool DENS, bool EPI>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
     __shared__ SharedStorage sm;
@@ -485,33 +497,34 @@ __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(co
     }
     __syncthreads();
     if (warp == kConsumerWarps) producer(a, sm, lane);
-    else                        consumer<PACKED, DENS>(a, sm, warp, lane);
+    else                        consumer<PACKED, DENS, EPI>(a, sm, warp, lane);
 }
 
 typedef void (*direct_fn)(const AccelArgs);
-static direct_fn pick_kernel(int variant, bool dens)
+static direct_fn pick_kernel(int variant, bool dens, bool epi)      // dens and epi are separate entry points
 {
-    if (variant == 0) return dens ? direct_kernel<true, true> : direct_kernel<true, false>;
-    return dens ? direct_kernel<false, true> : direct_kernel<false, false>;
+    if (variant == 0) return dens ? direct_kernel<true, true, false> : (epi ? direct_kernel<true, false, true> : direct_kernel<true, false, false>);
+    return dens ? direct_kernel<false, true, false> : (epi ? direct_kernel<false, false, true> : direct_kernel<false, false, false>);
 }
 
 int accel_max_ctas_per_sm(int variant)
 {
     int nb = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick_kernel(variant, false), kAccelThreads, 0);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick_kernel(variant, false, false), kAccelThreads, 0);
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
 
-// rho == NULL: forces only.  b is the density kernel radius in box units (validated by the caller).
-int launch_accel(nf_plan *p, float *acc, float *rho, double b)
+// rho == NULL: no density.  b is the density kernel radius in box units (validated by the caller).
+// vel / amax_cell: optional fused epilogue (kick by dt, per-cell maximum acceleration).
+int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, double dt, float *amax_cell)
 {
     cudaStream_t st = p->stream;
     p->have_accel_time = false;
     p->launches_accel = 0;
     if (p->n == 0 || p->n_units == 0) return NF_OK;
     const bool dens = rho != nullptr;
-    direct_fn fn = pick_kernel(p->variant, dens);
+    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr);
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
     if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
@@ -528,6 +541,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b)
     a.acc = acc;
     a.fastpath = p->fastpath;
     a.rho = rho; a.dens_nb2 = 0.f; a.dens_thr2 = 0.f; a.dens_mode = 0;
+    a.vel = vel; a.dt = (float)dt; a.amax = reinterpret_cast<uint32_t *>(amax_cell);
     if (dens) {
         const double bs = b * p->k.scale;                       // scaled units
         const double margin = 4.0 * 1.2e-7 * p->k.L * p->k.scale;   // as for the spline: float32 rounding of the coordinates
@@ -537,6 +551,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b)
     }
     NF_CUDA_OK(cudaEventRecord(p->ev[2], st));
     NF_CUDA_OK(cudaMemsetAsync(a.counter, 0, 4, st));
+    if (amax_cell) NF_CUDA_OK(cudaMemsetAsync(amax_cell, 0, 4 * (size_t)p->k.ncells, st));
     fn<<<(unsigned)grid, kAccelThreads, 0, st>>>(a);
     NF_CUDA_OK(cudaGetLastError());
     NF_CUDA_OK(cudaEventRecord(p->ev[3], st));

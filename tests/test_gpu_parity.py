@@ -386,3 +386,85 @@ def test_density_errors_and_empty():
         p.bin(torch.zeros((0, 3), device="cuda"))
         a, r = p.accel_density(0.1)
         assert a.shape == (0, 3) and r.shape == (0,)
+
+
+# ---------------------------------------------------------------- fused epilogue: kick + per-cell max |a| (NEXT 2)
+def kick_check(oracle_mod, pos_cpu, cpd, L, eps, dt, R=2, v0=None, what=""):
+    import paper_2110_11398_b200 as nf
+    pos = pos_cpu.numpy()
+    n = pos.shape[0]
+    v0 = torch.zeros((n, 3)) if v0 is None else v0
+    vel = v0.clone().cuda()
+    with nf.Plan(cpd, L, eps, R) as plan:
+        plan.bin(pos_cpu.cuda())
+        acc, amax = plan.accel_kick(vel, dt)
+        acc0 = plan.accel()
+        vel2 = v0.clone().cuda()
+        none_acc, amax2 = plan.accel_kick(vel2, dt, store_acc=False)           # accelerations not stored
+        torch.cuda.synchronize()
+    assert none_acc is None and torch.equal(vel, vel2) and torch.equal(amax, amax2)
+    assert torch.equal(acc, acc0)                                              # the epilogue does not change the forces
+    bn = oracle_mod.bin_particles(pos, cpd, L)
+    a_ref = oracle_mod.accel(pos, cpd, L, eps, R, binning=bn)
+    st = assert_parity(acc.cpu().numpy().astype(np.float64), a_ref, what)
+    # kick: the velocity change against a_ref dt, same tolerance as the accelerations, plus the float32
+    # rounding of the updated velocity (one FMA: half an ulp of v)
+    v_ref = oracle_mod.kick(v0.numpy(), a_ref, dt)
+    v_gpu = vel.cpu().numpy().astype(np.float64)
+    num = np.linalg.norm(v_gpu - v_ref, axis=1)
+    den = np.linalg.norm(a_ref * dt, axis=1)
+    slack = 2.0 ** -23 * np.linalg.norm(v_ref, axis=1)
+    ok = num <= 1e-5 * den + slack
+    assert ok.mean() >= 0.999 and np.all(num <= 1e-3 * den + slack), f"{what}: kick"
+    # per-cell maximum |a|
+    m_ref = oracle_mod.cell_max_accel(a_ref, bn["cid"], cpd ** 3)
+    m_gpu = amax.cpu().numpy().astype(np.float64)
+    assert np.all((m_gpu == 0) == (bn["count"] == 0))
+    nz = m_ref > 0
+    err = np.abs(m_gpu[nz] - m_ref[nz]) / m_ref[nz]
+    assert np.quantile(err, 0.999) <= 1e-5 and err.max() <= 1e-3, f"{what}: cell max {err.max():.3e}"
+    return {"amax_max_err": float(err.max()), **st}
+
+
+@pytest.mark.parametrize("idx,n_side,cpd", [(1, 32, 9), (2, 48, 12), (4, 40, 10), (5, 40, 10)])
+def test_kick_scaled_configs(oracle_mod, idx, n_side, cpd):
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    g = torch.Generator().manual_seed(idx)
+    v0 = torch.randn((cfg.n, 3), generator=g) * 50.0
+    print(cfg.name, kick_check(oracle_mod, pos, cfg.cpd, cfg.L, cfg.eps, 1e-3, cfg.R, v0=v0, what=cfg.name))
+    kick_check(oracle_mod, pos, cfg.cpd, cfg.L, cfg.eps, -0.25, cfg.R, what=cfg.name + " v0=0, dt<0")
+
+
+def test_kick_golden_two_body_gpu():
+    """a = +-256 x, dt = 2^-10: v_x changes by +-1/4 exactly; the cell maximum is 256, every other cell 0."""
+    import paper_2110_11398_b200 as nf
+    pos = torch.tensor([[0.53125, 0.5625, 0.5625], [0.59375, 0.5625, 0.5625]])
+    vel = torch.tensor([[1.0, 2.0, 3.0], [-1.0, 0.5, 0.0]]).cuda()
+    with nf.Plan(8, 1.0, 1e-6, 2) as p:
+        p.bin(pos.cuda())
+        _, amax = p.accel_kick(vel, 2.0 ** -10)
+    v = vel.cpu().numpy()
+    assert np.abs(v - np.array([[1.25, 2.0, 3.0], [-1.25, 0.5, 0.0]])).max() <= 1e-6
+    m = amax.cpu().numpy()
+    assert abs(m[(4 * 8 + 4) * 8 + 4] - 256.0) <= 1e-3 and np.count_nonzero(m) == 1
+
+
+def test_kick_errors_and_empty():
+    import paper_2110_11398_b200 as nf
+    B = nf.binding
+    with nf.Plan(5, 1.0, 0.01, 2) as p:
+        with pytest.raises(nf.NFError) as e:
+            nf.nf_accel_kick(p._h, None, torch.zeros((3, 3), device="cuda"), 0.1, None)
+        assert e.value.code == B.NF_ERR_STATE
+        p.bin(torch.rand((100, 3), device="cuda"))
+        with pytest.raises(nf.NFError) as e:
+            nf.nf_accel_kick(p._h, None, None, 0.1, None)
+        assert e.value.code == B.NF_ERR_ARG
+        with pytest.raises(nf.NFError) as e:
+            p.accel_kick(torch.zeros((100, 3), device="cuda"), float("inf"))
+        assert e.value.code == B.NF_ERR_ARG
+        p.bin(torch.zeros((0, 3), device="cuda"))
+        a, m = p.accel_kick(torch.zeros((0, 3), device="cuda"), 0.1)
+        torch.cuda.synchronize()
+        assert a.shape == (0, 3) and not m.cpu().numpy().any()

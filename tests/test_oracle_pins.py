@@ -419,3 +419,43 @@ def test_density_invariants(oracle_mod):
     # b larger than R cell widths would truncate the sum: rejected (reading D2)
     with pytest.raises(oracle_mod.OracleError):
         oracle_mod.density(pos, 8, 1.0, 0.26, 2)
+
+
+# ---------------------------------------------------------------- kick and per-cell maximum acceleration
+def test_kick_and_cell_max_closed_forms(oracle_mod):
+    """Two particles 1/16 apart along x in cell (4,4,4) of an 8^3 grid: a = +-256 x (golden two-body case), so a kick by
+    dt = 2^-10 changes v_x by +-1/4 exactly and the cell maximum is 256; every other cell is empty (0)."""
+    pos = np.array([[0.53125, 0.5625, 0.5625], [0.59375, 0.5625, 0.5625]], np.float32)
+    a = oracle_mod.accel(pos, 8, 1.0, 1e-6, 2)
+    v0 = np.array([[1.0, 2.0, 3.0], [-1.0, 0.5, 0.0]])
+    v = oracle_mod.kick(v0, a, 2.0 ** -10)
+    assert np.array_equal(v, np.array([[1.25, 2.0, 3.0], [-1.25, 0.5, 0.0]]))
+    b = oracle_mod.bin_particles(pos, 8, 1.0)
+    m = oracle_mod.cell_max_accel(a, b["cid"], 512)
+    assert m[(4 * 8 + 4) * 8 + 4] == 256.0 and np.count_nonzero(m) == 1
+
+
+def test_kick_and_cell_max_invariants(oracle_mod):
+    rng = np.random.default_rng(21)
+    pos = rng.random((4000, 3), dtype=np.float32)
+    cpd = 6
+    b = oracle_mod.bin_particles(pos, cpd, 1.0)
+    a = oracle_mod.accel(pos, cpd, 1.0, 0.003, 2, binning=b)
+    v0 = rng.normal(size=(4000, 3))
+    dt = 1e-4
+    v = oracle_mod.kick(v0, a, dt)
+    # total momentum is conserved by the kick because the near-field forces sum to zero
+    assert np.abs((v - v0).sum(0)).max() <= 1e-12 * np.abs(a * dt).sum()
+    # brute-force per-cell maximum (pure Python), empty cells zero, attained by a member
+    m = oracle_mod.cell_max_accel(a, b["cid"], cpd ** 3)
+    norms = [math.sqrt(float(x @ x)) for x in a]
+    want = [0.0] * cpd ** 3
+    for i, c in enumerate(b["cid"]):
+        want[int(c)] = max(want[int(c)], norms[i])
+    assert np.allclose(m, want, rtol=1e-15, atol=0)
+    assert np.all((m == 0) == (b["count"] == 0))
+    # input-order shuffle leaves the per-cell maxima unchanged
+    perm = rng.permutation(4000)
+    b2 = oracle_mod.bin_particles(pos[perm], cpd, 1.0)
+    a2 = oracle_mod.accel(pos[perm], cpd, 1.0, 0.003, 2, binning=b2)
+    assert np.allclose(oracle_mod.cell_max_accel(a2, b2["cid"], cpd ** 3), m, rtol=1e-12)

@@ -41,6 +41,9 @@ def parse_args():
                     help="extra configs reported in 'per_config' (N=1 only, 3 warm-ups + 3 steps; config 5: 1 + 1); '' = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-density", action="store_true", help="skip the fused-density timing")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: 'replicas' (the contract: one GPU per problem, no sharding) or 'slabs' (ONE box split "
+                         "into x-slab ranges with an R-slab halo exchange inside every step: strong scaling)")
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--fastpath", type=int, default=None)
     ap.add_argument("--heavy-first", type=int, default=None)
@@ -388,6 +391,79 @@ def main_b200(args):
         dist.destroy_process_group()
 
 
+def main_slabs(args):
+    """one box of config --config sharded over the ranks by x-slabs.
+    A step = halo exchange (NCCL point-to-point) + nf_bin of own + halo particles + nf_accel of the owned sinks."""
+    import torch
+    import nf_inputs
+    import paper_2110_11398_b200 as nf
+    from paper_2110_11398_b200 import slabs
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = nf_inputs.config(args.config)
+    pos = nf_inputs.generate(cfg, device="cuda" if cfg.n > 20_000_000 else "cpu").cuda()   # same seed on every rank
+    first, cnt = slabs.slab_partition(cfg.cpd, world)[rank]
+    own = pos[((slabs.slab_of(pos, cfg.cpd, cfg.L) - first) % cfg.cpd) < cnt].contiguous()
+    del pos
+    torch.cuda.empty_cache()
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        apply_options(plan, args)
+        plan.set_sink_slabs(first, cnt)
+        acc = None
+
+        def step():
+            nonlocal acc
+            loc, n_own = slabs.halo_exchange(own, cfg.cpd, cfg.L, cfg.R, rank, world, dist)
+            if acc is None or acc.shape[0] != loc.shape[0]:
+                acc = torch.empty_like(loc)
+            plan.bin(loc)
+            plan.accel(acc)
+            return loc.shape[0]
+
+        for _ in range(args.warmup):
+            n_local = step()
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        with ClockSampler(local) as clk:
+            ev[0].record()
+            for _ in range(args.steps):
+                n_local = step()
+            ev[1].record()
+            torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t_total = ev[0].elapsed_time(ev[1])
+        st = plan.stats()
+    inter = torch.tensor([float(st["interactions"]), float(own.shape[0])], device="cuda", dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(inter)
+    (t_total,) = max_over_ranks([t_total], dist, "cuda")
+    if rank == 0:
+        I, n = int(inter[0].item()), int(inter[1].item())
+        line = {"metric": METRIC, "value": I * args.steps / (t_total / 1e3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": t_total / args.steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": cfg.name, "n": n, "cpd": cfg.cpd, "R": cfg.R, "eps": cfg.eps, "L": cfg.L,
+                           "interactions_per_step": I, "l2": "inputs exceed L2",
+                           "parallelism": f"x-slabs dp{world}, R-slab halo exchange every step (torch.distributed P2P over NCCL)",
+                           "rank0_local_particles": n_local},
+                "particle_updates_per_s": n * args.steps / (t_total / 1e3),
+                "gpu_launches": args.steps * (st["kernel_launches_bin"] + st["kernel_launches_accel"]),
+                "clocks": clk.summary()}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main_reference(args):
     """The reference arm of this tier is the oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -422,5 +498,7 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         main_reference(a)
+    elif a.decomp == "slabs":
+        main_slabs(a)
     else:
         main_b200(a)

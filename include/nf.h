@@ -127,6 +127,18 @@ int nf_accel_kick(nf_plan *plan, float *acc_dev, float *vel_dev, double dt, floa
 /* nf_destroy -- frees everything the plan allocated (never a caller workspace).  NULL-safe. */
 void nf_destroy(nf_plan *plan);
 
+/*
+ * nf_set_sink_slabs -- x-slab domain decomposition (the paper's parallel method: each node owns a contiguous
+ * range of slabs and needs "R loaded slabs on either side").  After this call only the
+ * particles whose cell has x index in {x_first, ..., x_first + n_slabs - 1} (mod cpd) are SINKS; every binned
+ * particle is still a source.  A rank bins its own slabs plus the R halo slabs of each x-neighbour and gets
+ * exactly the accelerations a whole-box plan would give its particles; rows of acc that belong to particles
+ * outside the sink slabs are not written, and nf_stats.interactions counts the owned sinks only.
+ * Takes effect at the next nf_bin (it invalidates the current binning).  Default: all slabs.
+ * Errors: NF_ERR_ARG unless 0 <= x_first < cpd and 1 <= n_slabs <= cpd.
+ */
+int nf_set_sink_slabs(nf_plan *plan, int x_first, int n_slabs);
+
 /* ---- host-buffer entry points (end-to-end path: the copies are part of the call) ------------- */
 
 /* Copies pos_host [n][3] to a plan-owned device buffer (async if pinned) and runs nf_bin on it. */

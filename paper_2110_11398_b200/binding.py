@@ -21,7 +21,7 @@ NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -
 _ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
 
 EXPORTS = [
-    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
 ]
@@ -66,6 +66,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_accel_density.argtypes = [vp, vp, vp, dbl]
     lib.nf_accel_kick.restype = i32
     lib.nf_accel_kick.argtypes = [vp, vp, vp, dbl, vp]
+    lib.nf_set_sink_slabs.restype = i32
+    lib.nf_set_sink_slabs.argtypes = [vp, i32, i32]
     lib.nf_destroy.restype = None
     lib.nf_destroy.argtypes = [vp]
     lib.nf_bin_host.restype = i32
@@ -164,6 +166,10 @@ def nf_accel_kick(plan: int, acc: torch.Tensor | None, vel: torch.Tensor | None,
     _check(_lib.nf_accel_kick(plan, pa, pv, float(dt), pm))
 
 
+def nf_set_sink_slabs(plan: int, x_first: int, n_slabs: int) -> None:
+    _check(_lib.nf_set_sink_slabs(plan, int(x_first), int(n_slabs)))
+
+
 def nf_bin_host(plan: int, pos_host: torch.Tensor) -> None:
     pos_host = _host_f32(pos_host, "pos_host")
     _check(_lib.nf_bin_host(plan, ctypes.c_void_p(pos_host.data_ptr()), pos_host.shape[0]))
@@ -259,6 +265,9 @@ class Plan:
 
     def set_option(self, key: str, value: int):
         nf_set_option(self._h, key, value)
+
+    def set_sink_slabs(self, x_first: int, n_slabs: int):
+        nf_set_sink_slabs(self._h, x_first, n_slabs)
 
     def bin(self, pos: torch.Tensor):
         self._use_current_stream()

@@ -145,6 +145,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     memset(p, 0, sizeof(*p));
     Consts &k = p->k;
     k.cpd = cpd; k.R = R; k.ncells = (uint32_t)cpd * cpd * cpd;
+    k.slab0 = 0; k.nslab = cpd;
     k.L = L; k.cell_w = L / cpd; k.inv_cell_w = (double)cpd / L;
     int e2 = 0;
     (void)std::frexp(k.cell_w, &e2);              // cell_w = m 2^e2, m in [0.5, 1)
@@ -211,6 +212,18 @@ int nf_set_workspace(nf_plan *p, void *dev_ptr, size_t bytes)
     if (p->arena && p->arena_owned) cudaFree(p->arena);
     p->arena = dev_ptr; p->arena_bytes = dev_ptr ? bytes : 0; p->arena_owned = false;
     p->ws_n = -1; p->binned = false;
+    return NF_OK;
+}
+
+int nf_set_sink_slabs(nf_plan *p, int x_first, int n_slabs)
+{
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (x_first < 0 || x_first >= p->k.cpd || n_slabs < 1 || n_slabs > p->k.cpd) {
+        set_error("sink slabs: need 0 <= x_first < cpd and 1 <= n_slabs <= cpd (got %d, %d)", x_first, n_slabs);
+        return NF_ERR_ARG;
+    }
+    p->k.slab0 = x_first; p->k.nslab = n_slabs;
+    p->binned = false;                       // the work units depend on it
     return NF_OK;
 }
 

@@ -265,7 +265,8 @@ __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t 
             }
         }
         src_out[c] = src;
-        mine = (unsigned long long)count[c] * src;
+        int rel = cx - k.slab0; rel += rel < 0 ? cpd : 0;
+        if (rel < k.nslab) mine = (unsigned long long)count[c] * src;      // sinks of the owned slabs only
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(0xffffffffu, mine, o);
@@ -285,7 +286,8 @@ __global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t 
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
     const uint32_t ncol = offset[(size_t)(col + 1) * k.cpd] - offset[(size_t)col * k.cpd];
-    nunits[col] = (ncol + kChunk - 1) / kChunk;
+    int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
+    nunits[col] = rel < k.nslab ? (ncol + kChunk - 1) / kChunk : 0u;            // columns outside the sink slabs: sources only
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
@@ -297,6 +299,8 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
     const uint32_t *off = offset + (size_t)col * k.cpd;
     const uint32_t *sc = src + (size_t)col * k.cpd;
+    int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
+    if (rel >= k.nslab) return;
     const uint32_t c_begin = off[0], c_end = off[k.cpd];
     uint32_t u = ubase[col];
     int z = 0;

@@ -63,6 +63,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
 
 struct Consts {          // everything the kernels need about the problem, by value
     int cpd, R;
+    int slab0, nslab;               // sink slabs: cells with x index in {slab0, ..., slab0 + nslab - 1} mod cpd (default: all)
     uint32_t ncells;
     double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L
     double scale;                   // power of two with cell_w*scale in [1,2)

@@ -468,3 +468,56 @@ def test_kick_errors_and_empty():
         a, m = p.accel_kick(torch.zeros((0, 3), device="cuda"), 0.1)
         torch.cuda.synchronize()
         assert a.shape == (0, 3) and not m.cpu().numpy().any()
+
+
+# ---------------------------------------------------------------- x-slab decomposition (NEXT 3), ranks emulated one after another
+@pytest.mark.parametrize("idx,n_side,cpd,world", [(3, 40, 10, 2), (4, 40, 10, 3), (1, 32, 9, 4), (2, 48, 5, 2)])
+def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, world):
+    """Each emulated rank bins its slabs plus the halo its peers would send (slabs.select_for_peer, the function
+    halo_exchange ships) and computes its own sinks: bit-identical to the whole-box plan, interaction counts add up."""
+    import paper_2110_11398_b200 as nf
+    from paper_2110_11398_b200 import slabs
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos.cuda())
+        whole = plan.accel().cpu()
+        total = plan.stats()["interactions"]
+    sl = slabs.slab_of(pos, cfg.cpd, cfg.L)
+    parts = slabs.slab_partition(cfg.cpd, world)
+    owned = [pos[((sl - f) % cfg.cpd) < c].contiguous() for f, c in parts]
+    idx_owned = [torch.nonzero(((sl - f) % cfg.cpd) < c).squeeze(1) for f, c in parts]
+    got = torch.full_like(whole, float("nan"))
+    inter = 0
+    for r, (f, c) in enumerate(parts):
+        halos = [slabs.select_for_peer(owned[q], slabs.slab_of(owned[q], cfg.cpd, cfg.L), parts[r], cfg.cpd, cfg.R)
+                 for q in range(world) if q != r]
+        local = torch.cat([owned[r]] + halos).contiguous()
+        with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+            plan.set_sink_slabs(f, c)
+            plan.bin(local.cuda())
+            acc = torch.full((local.shape[0], 3), 7.0, device="cuda")
+            plan.accel(acc)
+            torch.cuda.synchronize()
+            inter += plan.stats()["interactions"]
+        acc = acc.cpu()
+        assert torch.all(acc[owned[r].shape[0]:] == 7.0)              # halo rows are not written
+        got[idx_owned[r]] = acc[:owned[r].shape[0]]
+    assert torch.equal(got, whole)
+    assert inter == total
+    ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
+    assert_parity(got.numpy().astype(np.float64), ref, f"{cfg.name} in {world} slab ranges")
+
+
+def test_sink_slab_errors():
+    import paper_2110_11398_b200 as nf
+    with nf.Plan(6, 1.0, 0.01, 2) as p:
+        for bad in ((-1, 2), (6, 1), (0, 0), (0, 7)):
+            with pytest.raises(nf.NFError) as e:
+                p.set_sink_slabs(*bad)
+            assert e.value.code == nf.binding.NF_ERR_ARG
+        p.bin(torch.rand((50, 3), device="cuda"))
+        p.set_sink_slabs(4, 3)                                        # wraps: slabs 4, 5, 0
+        with pytest.raises(nf.NFError) as e:                          # the binning was invalidated
+            p.accel()
+        assert e.value.code == nf.binding.NF_ERR_STATE

@@ -123,8 +123,21 @@ int nfo_bin(const float *pos, int64_t n, int cpd, double L,
     return NFO_OK;
 }
 
-/* Acceleration on input particle i (float64), by the definition O4. */
-static void nfo_one_sink(const float *pos, int cpd, double L, double eps, int R,
+/*
+ * The comparison law of the paper: "the commonly used Plummer softening based on the potential
+ * 1/sqrt(r^2 + eps^2), which converges only quadratically to the correct large-scale force law"
+ * (sec. 5.2).  Force on the sink: d * (r^2 + eps^2)^(-3/2); eps is the Plummer length itself.
+ * r = 0 contributes 0 (d = 0); eps = 0 is the Newtonian law with the r = 0 convention of reading C5.
+ */
+double nfo_kernel_plummer(double r, double eps)
+{
+    if (r == 0.0) return 0.0;
+    double s = r * r + eps * eps;
+    return 1.0 / (s * sqrt(s));
+}
+
+/* Acceleration on input particle i (float64), by the definition O4.  kind 0: spline (the method), 1: Plummer. */
+static void nfo_one_sink(const float *pos, int cpd, double L, double eps, int R, int kind,
                          const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
                          int64_t i, double *a_out)
 {
@@ -150,7 +163,7 @@ static void nfo_one_sink(const float *pos, int cpd, double L, double eps, int R,
             double dz = (double)pos[3 * j + 2] - zi + wz * L;
             double r2 = dx * dx + dy * dy + dz * dz;
             if (r2 == 0.0) continue;
-            double K = nfo_kernel(sqrt(r2), eps);
+            double K = kind == 1 ? nfo_kernel_plummer(sqrt(r2), eps) : nfo_kernel(sqrt(r2), eps);
             ax += dx * K; ay += dy * K; az += dz * K;
         }
     }
@@ -163,10 +176,11 @@ static void nfo_one_sink(const float *pos, int cpd, double L, double eps, int R,
  *   acc    [m][3] float64 out, row k belongs to sinks[k] (or to input particle k if sinks==NULL)
  * The binning arrays must come from nfo_bin on the same pos/cpd/L.
  */
-int nfo_accel(const float *pos, int64_t n, int cpd, double L, double eps, int R,
-              const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
-              const int64_t *sinks, int64_t m, double *acc)
+int nfo_accel_kind(const float *pos, int64_t n, int cpd, double L, double eps, int R, int kind,
+                   const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
+                   const int64_t *sinks, int64_t m, double *acc)
 {
+    if (kind != 0 && kind != 1) return NFO_ERR_ARG;
     if (nfo_check_args(cpd, L, eps, R) != NFO_OK || n < 0 || m < 0) return NFO_ERR_ARG;
     if (!sinks && m != n) return NFO_ERR_ARG;
     int bad = 0;
@@ -174,9 +188,16 @@ int nfo_accel(const float *pos, int64_t n, int cpd, double L, double eps, int R,
     for (int64_t k = 0; k < m; k++) {
         int64_t i = sinks ? sinks[k] : k;
         if (i < 0 || i >= n) { bad |= 1; continue; }
-        nfo_one_sink(pos, cpd, L, eps, R, cid, offset, perm, i, acc + 3 * k);
+        nfo_one_sink(pos, cpd, L, eps, R, kind, cid, offset, perm, i, acc + 3 * k);
     }
     return bad ? NFO_ERR_ARG : NFO_OK;
+}
+
+int nfo_accel(const float *pos, int64_t n, int cpd, double L, double eps, int R,
+              const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
+              const int64_t *sinks, int64_t m, double *acc)
+{
+    return nfo_accel_kind(pos, n, cpd, L, eps, R, 0, cid, offset, perm, sinks, m, acc);
 }
 
 /*

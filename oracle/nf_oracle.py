@@ -42,6 +42,10 @@ def _load():
         lib.nfo_kernel.argtypes = [f64, f64]
         lib.nfo_bin.restype = i32
         lib.nfo_bin.argtypes = [vp, i64, i32, f64, vp, vp, vp, vp]
+        lib.nfo_kernel_plummer.restype = f64
+        lib.nfo_kernel_plummer.argtypes = [f64, f64]
+        lib.nfo_accel_kind.restype = i32
+        lib.nfo_accel_kind.argtypes = [vp, i64, i32, f64, f64, i32, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_accel.restype = i32
         lib.nfo_accel.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_density.restype = i32
@@ -69,8 +73,10 @@ def num_threads() -> int:
     return int(_load().nfo_num_threads())
 
 
-def kernel(r: float, eps: float) -> float:
+def kernel(r: float, eps: float, softening: str = "spline") -> float:
     """K(r): the acceleration on a sink from a unit-mass source at displacement d is d*K(|d|)."""
+    if softening == "plummer":
+        return float(_load().nfo_kernel_plummer(float(r), float(eps)))
     return float(_load().nfo_kernel(float(r), float(eps)))
 
 
@@ -89,8 +95,10 @@ def bin_particles(pos, cpd: int, L: float):
     return {"cid": cid, "count": count, "offset": offset, "perm": perm}
 
 
-def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=None) -> np.ndarray:
-    """float64 accelerations [m][3]; ``sinks`` = input indices to evaluate (default: all, input order)."""
+def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=None, softening: str = "spline") -> np.ndarray:
+    """float64 accelerations [m][3]; ``sinks`` = input indices to evaluate (default: all, input order).
+    ``softening``: "spline" (the method) or "plummer" (the paper's comparison law)."""
+    kind = {"spline": 0, "plummer": 1}[softening]
     pos = _pos32(pos)
     n = pos.shape[0]
     if binning is None:
@@ -101,7 +109,7 @@ def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=N
         sinks = np.ascontiguousarray(sinks, dtype=np.int64)
         sp, m = sinks.ctypes.data, sinks.shape[0]
     acc = np.zeros((m, 3), np.float64)
-    rc = _load().nfo_accel(pos.ctypes.data, n, cpd, float(L), float(eps), int(R),
+    rc = _load().nfo_accel_kind(pos.ctypes.data, n, cpd, float(L), float(eps), int(R), kind,
                            binning["cid"].ctypes.data, binning["offset"].ctypes.data,
                            binning["perm"].ctypes.data, sp, m, acc.ctypes.data)
     _check(rc, "nfo_accel")

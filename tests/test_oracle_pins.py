@@ -459,3 +459,44 @@ def test_kick_and_cell_max_invariants(oracle_mod):
     b2 = oracle_mod.bin_particles(pos[perm], cpd, 1.0)
     a2 = oracle_mod.accel(pos[perm], cpd, 1.0, 0.003, 2, binning=b2)
     assert np.allclose(oracle_mod.cell_max_accel(a2, b2["cid"], cpd ** 3), m, rtol=1e-12)
+
+
+# ---------------------------------------------------------------- Plummer comparison law
+def test_plummer_kernel_closed_forms(oracle_mod):
+    """Force d (r^2 + eps^2)^(-3/2) of the potential 1/sqrt(r^2 + eps^2): a 3-4-5 case, the centre, the force
+    maximum at r = eps/sqrt(2) (F = 2/(3 sqrt(3) eps^2), textbook) and the quadratic approach to Newton that the
+    paper objects to ("converges only quadratically", "percent-level ... even at 15 eps")."""
+    K = lambda r, e: oracle_mod.kernel(r, e, "plummer")
+    assert math.isclose(K(3 / 64, 1 / 16) * 3 / 64, 98.304, rel_tol=1e-15)        # (3/64) / (5/64)^3
+    eps = 0.01
+    assert math.isclose(K(1e-12, eps), eps ** -3, rel_tol=1e-12) and K(0.0, eps) == 0.0
+    rs = np.linspace(0.2 * eps, 3 * eps, 20001)
+    F = np.array([r * K(r, eps) for r in rs])
+    assert abs(rs[F.argmax()] - eps / math.sqrt(2)) < 2e-4 * eps
+    assert math.isclose(F.max(), 2 / (3 * math.sqrt(3) * eps ** 2), rel_tol=1e-7)
+    for m in (15.0, 30.0, 100.0):
+        r = m * eps
+        deficit = 1.0 - K(r, eps) * r ** 3
+        assert math.isclose(deficit, 1.5 / m ** 2, rel_tol=3.0 / m ** 2 + 1e-9)
+    assert 0.005 < 1.0 - K(15 * eps, eps) * (15 * eps) ** 3 < 0.01                # "percent-level" at 15 eps
+    assert K(0.3, 0.0) == pytest.approx(0.3 ** -3, rel=1e-15)                     # eps = 0: Newtonian
+
+
+@pytest.mark.parametrize("cpd,R,n,eps", [(6, 2, 400, 0.01), (7, 2, 300, 0.05), (4, 1, 200, 0.0)])
+def test_plummer_brute_force(oracle_mod, cpd, R, n, eps):
+    """Independent route: all pairs, minimum image, explicit cell-offset mask, Plummer law in numpy."""
+    rng = np.random.default_rng(n)
+    pos = rng.random((n, 3), dtype=np.float32)
+    a = oracle_mod.accel(pos, cpd, 1.0, eps, R, softening="plummer")
+    p = pos.astype(np.float64)
+    c = np.minimum(np.floor(p * cpd).astype(int), cpd - 1)
+    m = np.abs(c[None] - c[:, None]) % cpd
+    near = np.minimum(m, cpd - m).max(-1) <= R          # wrapped cell offset, max-norm (cpd >= 2R+2: minimum image)
+    d = p[None] - p[:, None]
+    d -= np.round(d)
+    s = (d ** 2).sum(-1) + eps ** 2
+    with np.errstate(divide="ignore"):
+        k = np.where(near & ((d ** 2).sum(-1) > 0), s ** -1.5, 0.0)
+    ref = (d * k[..., None]).sum(1)
+    np.testing.assert_allclose(a, ref, rtol=1e-9, atol=1e-9 * np.abs(ref).max())
+    assert np.abs(a.sum(0)).max() <= 1e-10 * np.abs(a).sum()

@@ -188,6 +188,9 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
+ *   "softening"    0 = the compact spline of the method (default); 1 = Plummer softening, force
+ *                  d (r^2 + eps^2)^(-3/2) with eps the plan's length: the law the paper compares against
+ *                  ("converges only quadratically to the correct large-scale force law")
  */
 int nf_set_option(nf_plan *plan, const char *key, long long value);
 

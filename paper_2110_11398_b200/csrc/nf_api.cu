@@ -364,6 +364,13 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
     if (!strcmp(key, "variant") && (v == 0 || v == 1)) { p->variant = (int)v; return NF_OK; }
     if (!strcmp(key, "fastpath") && (v == 0 || v == 1)) { p->fastpath = (int)v; return NF_OK; }
     if (!strcmp(key, "heavy_first") && (v == 0 || v == 1)) { p->heavy_first = (int)v; p->binned = false; return NF_OK; }
+    if (!strcmp(key, "softening") && (v == 0 || v == 1)) {
+        // 0: the spline of the method; 1: the Plummer comparison law.  eps = 0 is Newtonian either way.
+        const double es = p->eps * p->k.scale;
+        p->k.plummer = (v == 1 && p->eps > 0.0) ? 1 : 0;
+        p->k.tiny = p->k.plummer ? (float)(es * es) : 1e-36f;
+        return NF_OK;
+    }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
     set_error("unknown option or bad value: %s = %lld", key, v);
     return NF_ERR_ARG;

@@ -318,7 +318,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
                 if (jy < 0) { jy += cpd; wy = -k.L; } else if (jy >= cpd) { jy -= cpd; wy = k.L; }
                 const float Dy = (float)(((double)(float)((double)jy * k.cell_w) + wy - ocy) * k.scale);
                 const uint32_t row = ((uint32_t)jx * cpd + jy) * cpd;
-                const int soft_mode = !(k.fast_ok && a.fastpath) ? 2 : ((ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1) ? 1 : 0);
+                const int soft_mode = k.plummer ? 0 : !(k.fast_ok && a.fastpath) ? 2 : ((ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1) ? 1 : 0);
                 for (int jb = jlo; jb <= jhi; jb += 32) {
                     // the warp fetches the padded offsets of up to 32 cells of the run at once
                     const int jl = jb + lane;

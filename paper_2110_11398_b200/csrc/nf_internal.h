@@ -69,6 +69,7 @@ struct Consts {          // everything the kernels need about the problem, by va
     double scale;                   // power of two with cell_w*scale in [1,2)
     float A, B, C;                  // spline in scaled units: t(r) = A + B r + C r^2
     float tiny;
+    int plummer;                    // 1: Plummer law d (r^2 + eps^2)^-3/2 (tiny = eps^2, no spline anywhere)
     int fast_ok;                    // eps_s <= 0.999 cell_w: cells with max-norm offset >= 2 are pure Newtonian
     double out_scale;               // scale^2
     float w_scaled;                 // cell width in scaled units, in [1,2)

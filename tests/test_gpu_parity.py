@@ -521,3 +521,27 @@ def test_sink_slab_errors():
         with pytest.raises(nf.NFError) as e:                          # the binning was invalidated
             p.accel()
         assert e.value.code == nf.binding.NF_ERR_STATE
+
+
+# ---------------------------------------------------------------- Plummer comparison law (NEXT 4)
+@pytest.mark.parametrize("idx,n_side,cpd,variant", [(1, 32, 9, 0), (4, 40, 10, 0), (5, 40, 10, 1)])
+def test_plummer_softening(oracle_mod, idx, n_side, cpd, variant):
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    out = gpu_run(pos, cfg.cpd, cfg.L, cfg.eps, cfg.R, options={"softening": 1, "variant": variant})
+    ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R, softening="plummer")
+    print(cfg.name, "plummer", assert_parity(out["acc"], ref, cfg.name + " plummer"))
+    spline = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
+    assert rel_errors(out["acc"], spline).max() > 1e-4            # it really is a different law
+
+
+def test_plummer_two_body_and_large_eps(oracle_mod):
+    """3-4-5 case: |a| = 98.304; eps of several cell widths (no compact support: every stencil cell is softened)."""
+    pos = torch.tensor([[0.5, 0.5625, 0.5625], [0.5 + 3 / 64, 0.5625, 0.5625]])
+    a = gpu_run(pos, 8, 1.0, 1 / 16, 2, options={"softening": 1})["acc"]
+    assert np.abs(a - np.array([[98.304, 0, 0], [-98.304, 0, 0]])).max() <= 2e-5
+    g = torch.Generator().manual_seed(5)
+    p = torch.rand((4000, 3), generator=g)
+    for eps in (0.3, 0.0):
+        out = gpu_run(p, 6, 1.0, eps, 2, options={"softening": 1})
+        assert_parity(out["acc"], oracle_mod.accel(p.numpy(), 6, 1.0, eps, 2, softening="plummer"), f"plummer eps={eps}")

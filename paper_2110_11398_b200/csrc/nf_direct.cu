@@ -67,15 +67,20 @@ __device__ __forceinline__ void mbar_init(void *bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
+__device__ __forceinline__ bool mbar_try(uint32_t a, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    return ok != 0;
+}
+// A warp that has to wait (the producer running ahead, a consumer warp without sinks in a ragged window) backs
+// off with nanosleep: a spinning try_wait loop costs issue slots that the working warps of the sub-partition need.
 __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
 {
     const uint32_t a = smem_u32(bar);
-    uint32_t ok;
-    do {
-        // the suspend-time hint parks the warp in hardware instead of spinning through issue slots
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity), "r"(0x989680u) : "memory");
-    } while (!ok);
+    if (mbar_try(a, parity)) return;
+    while (!mbar_try(a, parity)) __nanosleep(kWaitSleepNs);
 }
 __device__ __forceinline__ void mbar_arrive(void *bar)
 {

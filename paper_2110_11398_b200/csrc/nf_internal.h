@@ -31,6 +31,10 @@ constexpr int kStages        = NF_STAGES;         // TMA pipeline depth
 constexpr int kMaxPieces     = 24;                // source cells (table entries) per stage
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
 constexpr int kMinCtasPerSm  = NF_MIN_CTAS;       // register budget: 65536 / (kMinCtasPerSm * kAccelThreads) per thread
+#ifndef NF_WAIT_SLEEP_NS
+#define NF_WAIT_SLEEP_NS 400
+#endif
+constexpr unsigned kWaitSleepNs = NF_WAIT_SLEEP_NS;  // back-off of a waiting warp between mbarrier polls
 constexpr float kDummy       = 36028797018963968.0f;        // 2^55: pad-slot coordinate, contributes exactly 0
 
 // ---- radix sort shape ----------------------------------------------------------------------

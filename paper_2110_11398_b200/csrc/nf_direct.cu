@@ -105,10 +105,8 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 // ---- pair bodies -------------------------------------------------------------------------------
 struct SoftCoef { float A, B, C, tiny, soft_r2, nb2; };   // nb2 = -1/b^2 of the density kernel
 
-// two sources (packed) against one sink: 14 (spline) / 11 (Newtonian) FP32-pipe instructions per pair of
-// interactions, plus 2 MUFU.RSQ and, spline only, 2 FMNMX.  The kernel uses the Newtonian instance; the
-// spline of the packed path is pair_head / pair_spline below.
-template <bool SOFT>
+// two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
+// (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ
 __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
                                           const float2 nz, const SoftCoef &c, float2 &ax, float2 &ay, float2 &az)
 {
@@ -120,14 +118,7 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
     ri.x = rsqrt_approx(r2.x);
     ri.y = rsqrt_approx(r2.y);
     const float2 ri2 = __fmul2_rn(ri, ri);
-    float2 k = __fmul2_rn(ri2, ri);
-    if (SOFT) {
-        const float2 r = __fmul2_rn(r2, ri);                // t = (C r + B) r + A: one register constant per FFMA2
-        float2 t = __ffma2_rn(r, make_float2(c.C, c.C), make_float2(c.B, c.B));
-        t = __ffma2_rn(t, r, make_float2(c.A, c.A));
-        k.x = fminf(k.x, t.x);
-        k.y = fminf(k.y, t.y);
-    }
+    const float2 k = __fmul2_rn(ri2, ri);
     ax = __ffma2_rn(k, dx, ax);
     ay = __ffma2_rn(k, dy, ay);
     az = __ffma2_rn(k, dz, az);
@@ -203,8 +194,8 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 {
     if (PACKED && MODE == 0) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        interact2<false>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
-        interact2<false>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
     } else if (PACKED) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
         float2 dxa, dya, dza, r2a, ria, ka, dxb, dyb, dzb, r2b, rib, kb;

@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...)
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Carve the arena.  Called with base == NULL to get the size only.
-size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells)
+size_t carve(Workspace &ws, void *base, long long n, int cpd)
 {
     size_t off = 0;
     char *b = (char *)base;
@@ -33,10 +33,10 @@ size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells)
         return p;
     };
     const size_t N = (size_t)(n > 0 ? n : 0);
-    const size_t C = ncells;
+    const size_t C = (size_t)cpd * cpd * cpd;
     const size_t nonempty = N < C ? N : C;
     const size_t pmax = N + 3 * nonempty + 8;
-    const size_t ncol = (size_t)std::llround(std::cbrt((double)C)) * (size_t)std::llround(std::cbrt((double)C));
+    const size_t ncol = (size_t)cpd * cpd;
     const size_t umax = (N < ncol ? N : ncol) + N / kChunk + 2;    // every column ends with one ragged window
     const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
     const size_t sort_blocks = (nsort + kSortTile - 1) / kSortTile + 1;
@@ -86,9 +86,9 @@ static int ensure_device(nf_plan *p)
 static int ensure_workspace(nf_plan *p, long long n)
 {
     Workspace tmp;
-    size_t need = carve(tmp, nullptr, n, p->k.ncells);
+    size_t need = carve(tmp, nullptr, n, p->k.cpd);
     if (p->arena && p->arena_bytes >= need) {
-        if (p->ws_n != n) { carve(p->ws, p->arena, n, p->k.ncells); p->ws_n = n; }
+        if (p->ws_n != n) { carve(p->ws, p->arena, n, p->k.cpd); p->ws_n = n; }
         return NF_OK;
     }
     if (p->arena && !p->arena_owned) {
@@ -104,7 +104,7 @@ static int ensure_workspace(nf_plan *p, long long n)
         return NF_ERR_NOMEM;
     }
     p->arena = a; p->arena_bytes = need; p->arena_owned = true;
-    carve(p->ws, p->arena, n, p->k.ncells);
+    carve(p->ws, p->arena, n, p->k.cpd);
     p->ws_n = n;
     return NF_OK;
 }
@@ -202,7 +202,7 @@ size_t nf_workspace_bytes(const nf_plan *p, long long n)
 {
     if (!p || n < 0) return 0;
     Workspace tmp;
-    return carve(tmp, nullptr, n, p->k.ncells);
+    return carve(tmp, nullptr, n, p->k.cpd);
 }
 
 int nf_set_workspace(nf_plan *p, void *dev_ptr, size_t bytes)

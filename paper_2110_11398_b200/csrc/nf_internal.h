@@ -110,7 +110,7 @@ struct nf_plan {
 
 namespace nf {
 void set_error(const char *fmt, ...);
-size_t carve(Workspace &ws, void *base, long long n, uint32_t ncells);   // base may be NULL (size only)
+size_t carve(Workspace &ws, void *base, long long n, int cpd);   // base may be NULL (size only)
 int  launch_bin(nf_plan *p, const float *pos, long long n);             // S1-S5 (nf_bin.cu)
 int  launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, double dt, float *amax_cell);   // S6-S7 (nf_direct.cu)
 int  accel_max_ctas_per_sm(int variant);

@@ -152,6 +152,10 @@ struct Partial {
 };
 
 constexpr uint32_t kFull = 0xffffffffu;
+#ifndef NF_UNROLL_SOFT
+#define NF_UNROLL_SOFT 2
+#endif
+constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable piece loop
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
 
 // Newtonian part of two packed interactions: d, r^2, 1/r and k = r^-3
@@ -231,8 +235,13 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
 {
     const float4 *__restrict__ py = px + kTileAlloc / 4;
     const float4 *__restrict__ pz = py + kTileAlloc / 4;
+    if (MODE == 0) {
 #pragma unroll 2
-    for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+        for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+    } else {
+#pragma unroll kUnrollSoft
+        for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+    }
     for (int j = nmin; j < nmax; j++) {
         if (MODE >= 1 && PACKED) {                    // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;

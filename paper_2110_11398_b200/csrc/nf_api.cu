@@ -125,6 +125,44 @@ static int ensure_stage(nf_plan *p, long long n)
     return NF_OK;
 }
 
+// Softening constants of the pair bodies.  kind 0: the compact spline (readings C2/C3); kind 1: Plummer.
+static int set_softening(nf_plan *p, int kind)
+{
+    Consts &k = p->k;
+    const double eps = p->eps, L = k.L;
+    const double es = 2.16 * eps * k.scale;       // spline radius in scaled units
+    k.w_scaled = (float)(k.cell_w * k.scale);
+    if (kind == 1 && eps > 0.0) {
+        // d (r^2 + eps^2)^-3/2: the Newtonian body with eps^2 in place of the tiny r^2 offset; the spline never
+        // applies (t = 3e38 >= k, and no r^2 is below soft_r2 = 0)
+        const double ep = eps * k.scale;
+        k.plummer = 1;
+        k.tiny = (float)(ep * ep);
+        k.A = 3.0e38f; k.B = 0.f; k.C = 0.f;
+        k.fast_ok = 1; k.soft_thr2 = 0.f; k.soft_r2 = 0.f;
+        return NF_OK;
+    }
+    k.plummer = 0;
+    k.tiny = 1e-36f;
+    if (eps == 0.0) {
+        k.A = 3.0e38f; k.B = 0.f; k.C = 0.f;      // min(r^-3, 3e38): only r = 0 is capped, and 3e38 * 0 = 0
+    } else {
+        const double A = 10.0 / (es * es * es), B = -15.0 / (es * es * es * es), C = 6.0 / (es * es * es * es * es);
+        if (!(std::fabs(C) < 1e37) || !(std::fabs(B) < 1e37) || !(A < 1e37)) {
+            set_error("eps = %g is too small relative to the cell width %g for float32 spline coefficients; use eps = 0", eps, k.cell_w);
+            return NF_ERR_ARG;
+        }
+        k.A = (float)A; k.B = (float)B; k.C = (float)C;
+    }
+    k.fast_ok = (2.16 * eps <= 0.999 * k.cell_w) ? 1 : 0;
+    // cell-relative coordinates carry the float32 rounding of the position and of the corner: <= 2^-23 L each
+    const double margin = 4.0 * 1.2e-7 * L * k.scale;
+    const double thr = es + margin;
+    k.soft_thr2 = (float)(thr * thr * 1.0001);
+    k.soft_r2 = (float)(es * es * 1.001 + 1e-30);     // eps = 0: only r = 0 (r^2 = tiny) is below it
+    return NF_OK;
+}
+
 }  // namespace nf
 
 using namespace nf;
@@ -151,28 +189,8 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     (void)std::frexp(k.cell_w, &e2);              // cell_w = m 2^e2, m in [0.5, 1)
     k.scale = std::ldexp(1.0, 1 - e2);            // cell_w * scale in [1, 2)
     k.out_scale = k.scale * k.scale;
-    k.tiny = 1e-36f;
-    const double es = 2.16 * eps * k.scale;       // spline radius in scaled units
-    if (eps == 0.0) {
-        k.A = 3.0e38f; k.B = 0.f; k.C = 0.f;      // min(r^-3, 3e38): only r = 0 is capped, and 3e38 * 0 = 0
-    } else {
-        const double A = 10.0 / (es * es * es), B = -15.0 / (es * es * es * es), C = 6.0 / (es * es * es * es * es);
-        if (!(std::fabs(C) < 1e37) || !(std::fabs(B) < 1e37) || !(A < 1e37)) {
-            set_error("eps = %g is too small relative to the cell width %g for float32 spline coefficients; use eps = 0", eps, k.cell_w);
-            delete p;
-            return nullptr;
-        }
-        k.A = (float)A; k.B = (float)B; k.C = (float)C;
-    }
-    k.fast_ok = (2.16 * eps <= 0.999 * k.cell_w) ? 1 : 0;
-    k.w_scaled = (float)(k.cell_w * k.scale);
-    {   // cell-relative coordinates carry the float32 rounding of the position and of the corner: <= 2^-23 L each
-        const double margin = 4.0 * 1.2e-7 * L * k.scale;
-        const double thr = es + margin;
-        k.soft_thr2 = (float)(thr * thr * 1.0001);
-        k.soft_r2 = (float)(es * es * 1.001 + 1e-30);     // eps = 0: only r = 0 (r^2 = tiny) is below it
-    }
     p->eps = eps;
+    if (set_softening(p, 0) != NF_OK) { delete p; return nullptr; }
     p->device = -1;
     p->stream = 0;
     p->ws_n = -1;
@@ -366,10 +384,7 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
     if (!strcmp(key, "heavy_first") && (v == 0 || v == 1)) { p->heavy_first = (int)v; p->binned = false; return NF_OK; }
     if (!strcmp(key, "softening") && (v == 0 || v == 1)) {
         // 0: the spline of the method; 1: the Plummer comparison law.  eps = 0 is Newtonian either way.
-        const double es = p->eps * p->k.scale;
-        p->k.plummer = (v == 1 && p->eps > 0.0) ? 1 : 0;
-        p->k.tiny = p->k.plummer ? (float)(es * es) : 1e-36f;
-        return NF_OK;
+        return set_softening(p, (int)v);
     }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
     set_error("unknown option or bad value: %s = %lld", key, v);

@@ -103,7 +103,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
-struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, done; };   // density: nb2 = -1/b^2, done = 1 + tiny/b^2 (r^2 carries +tiny)
+struct SoftCoef { float A, B, C, tiny, soft_r2, nb2; int plummer; };   // nb2 = -1/b^2 of the density kernel
 
 // two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
 // (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ
@@ -139,7 +139,10 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
         const float t = fmaf(fmaf(r, c.C, c.B), r, c.A);
         k = fminf(k, t);
     }
-    if (MODE == 2) rho += fmaxf(fmaf(r2, c.nb2, c.done), 0.0f);
+    if (MODE == 2) {                      // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
+        const float q2 = c.plummer ? fmaf(dx, dx, fmaf(dy, dy, dz * dz)) : r2;
+        rho += fmaxf(fmaf(q2, c.nb2, 1.0f), 0.0f);
+    }
     ax = fmaf(k, dx, ax);
     ay = fmaf(k, dy, ay);
     az = fmaf(k, dz, az);
@@ -182,7 +185,7 @@ __device__ __forceinline__ void pair_spline(const float2 r2, const float2 ri, co
 // kernel density weights of two packed interactions: rho += max(0, 1 - r^2/b^2)
 __device__ __forceinline__ void pair_density(const float2 r2, const SoftCoef &c, float2 &rho)
 {
-    float2 w = __ffma2_rn(r2, make_float2(c.nb2, c.nb2), make_float2(c.done, c.done));
+    float2 w = __ffma2_rn(r2, make_float2(c.nb2, c.nb2), make_float2(1.0f, 1.0f));
     w.x = fmaxf(w.x, 0.0f);
     w.y = fmaxf(w.y, 0.0f);
     rho = __fadd2_rn(rho, w);
@@ -211,6 +214,10 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
             pair_spline(r2b, rib, c, kb);
         }
         if (MODE == 2) {
+            if (c.plummer) {                  // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
+                r2a = __ffma2_rn(dxa, dxa, __ffma2_rn(dya, dya, __fmul2_rn(dza, dza)));
+                r2b = __ffma2_rn(dxb, dxb, __ffma2_rn(dyb, dyb, __fmul2_rn(dzb, dzb)));
+            }
             pair_density(r2a, c, f.rho);
             pair_density(r2b, c, f.rho);
         }
@@ -384,8 +391,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
 template <bool PACKED, bool DENS, bool EPI>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
 {
-    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f,
-                           DENS ? 1.0f - a.k.tiny * a.dens_nb2 : 1.0f};   // the Plummer option puts eps^2 into r^2: take it out of the weight
+    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f, a.k.plummer};
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;

@@ -143,7 +143,8 @@ int nf_set_sink_slabs(nf_plan *plan, int x_first, int n_slabs);
 
 /* Copies pos_host [n][3] to a plan-owned device buffer (async if pinned) and runs nf_bin on it. */
 int nf_bin_host(nf_plan *plan, const float *pos_host, long long n);
-/* Runs nf_accel into a plan-owned device buffer and copies it to acc_host [n][3]; synchronises. */
+/* Runs nf_accel into a plan-owned device buffer and copies it to acc_host [n][3]; synchronises.
+ * With restricted sink slabs the rows of particles outside them come back as zeros. */
 int nf_accel_host(nf_plan *plan, float *acc_host);
 
 /* ---- supporting exports (harness, tests; not part of the paper's problem statement) ---------- */

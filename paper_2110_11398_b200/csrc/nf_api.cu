@@ -317,6 +317,8 @@ int nf_accel_host(nf_plan *p, float *acc_host)
     if (!acc_host && p->n > 0) { set_error("null acc_host"); return NF_ERR_ARG; }
     int rc = ensure_stage(p, p->n);
     if (rc) return rc;
+    if (p->k.nslab < p->k.cpd && p->n > 0)        // rows outside the sink slabs are not computed: hand back zeros
+        NF_CUDA_OK(cudaMemsetAsync(p->acc_stage, 0, (size_t)p->n * 12, p->stream));
     rc = launch_accel(p, p->acc_stage, nullptr, 0.0, nullptr, 0.0, nullptr);
     if (rc) return rc;
     if (p->n > 0) NF_CUDA_OK(cudaMemcpyAsync(acc_host, p->acc_stage, (size_t)p->n * 12, cudaMemcpyDeviceToHost, p->stream));

@@ -105,3 +105,76 @@ def test_fuzz_against_oracle(oracle_mod, seed):
         m_ref = oracle_mod.cell_max_accel(acc.cpu().numpy(), b["cid"], cpd ** 3)         # max of the SAME float32 vectors
         m_gpu = amax.cpu().numpy().astype(np.float64)
         assert np.allclose(m_gpu, m_ref, rtol=2e-7, atol=0), what
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_fuzz_call_sequences(oracle_mod, seed):
+    """One plan driven through random sequences of calls (re-binning with other sizes, options flipped between
+    calls, sink slabs, lent workspace, host entry points): every result must equal what the oracle says for the
+    state the calls define."""
+    import paper_2110_11398_b200 as nf
+    from paper_2110_11398_b200 import slabs
+    rng = np.random.default_rng(5000 + seed)
+    R = int(rng.integers(1, 3))
+    cpd = int(rng.integers(2 * R + 2, 14))
+    L = float(rng.choice([1.0, 3.0]))
+    cell = L / cpd
+    eps = float(rng.choice([0.0, 0.01, 0.05])) * cell
+    with nf.Plan(cpd, L, eps, R) as plan:
+        if rng.integers(0, 2):
+            ws = torch.empty(plan.workspace_bytes(20000) + 256, dtype=torch.uint8, device="cuda")
+            plan.set_workspace(ws)
+        plummer, first, cnt = False, 0, cpd
+        for step in range(6):
+            n = int(rng.choice([1, 50, 700, 5000, 20000]))
+            pos = _positions(rng, KINDS[int(rng.integers(0, 4))], n, L)
+            n = pos.shape[0]
+            if rng.integers(0, 2):
+                plummer = bool(rng.integers(0, 2))
+                plan.set_option("softening", int(plummer))
+            if rng.integers(0, 2):
+                plan.set_option("variant", int(rng.integers(0, 2)))
+            if rng.integers(0, 3) == 0:
+                first, cnt = int(rng.integers(0, cpd)), int(rng.integers(1, cpd + 1))
+                plan.set_sink_slabs(first, cnt)
+            what = f"seed {seed} step {step}: n={n} cpd={cpd} R={R} eps={eps:.3g} plummer={plummer} slabs=({first},{cnt})"
+            own = (((slabs.slab_of(torch.from_numpy(pos), cpd, L) - first) % cpd) < cnt).numpy()
+            b = oracle_mod.bin_particles(pos, cpd, L)
+            ref = oracle_mod.accel(pos, cpd, L, eps, R, binning=b, softening="plummer" if plummer and eps > 0 else "spline")
+            mode = int(rng.integers(0, 4))
+            sentinel = 12345.0
+            if mode == 3:                                            # host entry points
+                ph = torch.from_numpy(pos).pin_memory()
+                ah = torch.full((n, 3), sentinel).pin_memory()
+                plan.bin_host(ph)
+                plan.accel_host(ah)
+                a = ah.numpy().astype(np.float64)
+            else:
+                plan.bin(torch.from_numpy(pos).cuda())
+                acc = torch.full((n, 3), sentinel, device="cuda")
+                if mode == 0:
+                    plan.accel(acc)
+                elif mode == 1:
+                    bw = 0.4 * cell
+                    _, rho = plan.accel_density(bw, acc)
+                    ref_rho = oracle_mod.density(pos, cpd, L, bw, R, binning=b)
+                    err = np.abs(rho.cpu().numpy().astype(np.float64) - ref_rho)[own] / ref_rho[own]
+                    assert err.size == 0 or err.max() <= 1e-5, what + " density"
+                else:
+                    vel = torch.ones((n, 3), device="cuda")
+                    _, amax = plan.accel_kick(vel, 0.25, acc)
+                    torch.cuda.synchronize()
+                    assert torch.equal(vel[torch.from_numpy(own).cuda()], (1.0 + acc * 0.25)[torch.from_numpy(own).cuda()]), what
+                    assert torch.all(vel[torch.from_numpy(~own).cuda()] == 1.0), what
+                torch.cuda.synchronize()
+                a = acc.cpu().numpy().astype(np.float64)
+            assert np.all(a[~own] == (0.0 if mode == 3 else sentinel)), what + ": rows outside the sink slabs"
+            if own.any():
+                scale = np.linalg.norm(ref[own], axis=1).max() + 1e-300
+                err = np.linalg.norm(a[own] - ref[own], axis=1)
+                assert err.max() <= 1e-4 * scale and np.quantile(err / (np.linalg.norm(ref[own], axis=1) + 1e-300), 0.99) <= 1e-4, what
+            st = plan.stats()
+            cnt3 = b["count"].astype(np.int64).reshape(cpd, cpd, cpd)
+            box = sum(np.roll(cnt3, (ox, oy, oz), (0, 1, 2)) for ox in range(-R, R + 1) for oy in range(-R, R + 1) for oz in range(-R, R + 1))
+            ownx = ((np.arange(cpd) - first) % cpd) < cnt
+            assert st["interactions"] == int((cnt3 * box)[ownx].sum()), what

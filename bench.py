@@ -221,6 +221,25 @@ def aggregate_value(world, interactions, steps, total_ms):
     return world * interactions * steps / (total_ms / 1e3)
 
 
+def occupancy_stats(plan, cfg):
+    """Realised cell occupancy of the workload and where the interactions sit; harness-side torch."""
+    import torch
+    cnt = plan.binning()["count"].to(torch.int64).reshape(cfg.cpd, cfg.cpd, cfg.cpd)
+    box = torch.zeros_like(cnt)
+    for ox in range(-cfg.R, cfg.R + 1):
+        for oy in range(-cfg.R, cfg.R + 1):
+            for oz in range(-cfg.R, cfg.R + 1):
+                box += torch.roll(cnt, (ox, oy, oz), (0, 1, 2))
+    inter = (cnt * box).reshape(-1)
+    top = max(1, inter.numel() // 100)
+    heavy = torch.topk(inter, top).values.sum().item()
+    c = cnt.reshape(-1)
+    return {"max_per_cell": int(c.max().item()), "median_per_cell": float(c.median().item()),
+            "mean_per_cell": float(c.double().mean().item()), "empty_cells": int((c == 0).sum().item()),
+            "interactions_check": int(inter.sum().item()),
+            "share_of_interactions_in_heaviest_1pct_cells": heavy / max(1, inter.sum().item())}
+
+
 def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, warmup=None):
     import torch
     import nf_inputs
@@ -246,6 +265,7 @@ def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, wa
         I = st["interactions"]
         out.update(stats=st, interactions=I, total_ms=total_ms, accel_ms=acc_ms, bin_ms=bin_ms, steps=steps,
                    l2="flushed between iterations (256 MiB write)" if flush is not None else "inputs exceed L2")
+        out["occupancy"] = occupancy_stats(plan, cfg)
         a = acc.double()
         out["sum_check"] = float((a.sum(0).abs().max() / a.abs().sum()).item())   # total force ~ 0 at any size
         if with_e2e and not args.no_density:
@@ -306,7 +326,7 @@ def summarise(r):
         "ms_per_step": t * 1e3, "ms_bin": statistics.mean(r["bin_ms"]), "ms_accel": ta * 1e3,
         "fp32_peak_frac_25flop": FLOPS_PER_INTERACTION * I / ta / 1e12 / peak,
         "fp32_peak_frac_26flop_paper": 26 * I / ta / 1e12 / peak,
-        "sum_check": r["sum_check"], "l2": r["l2"], "clocks": r["clocks"],
+        "sum_check": r["sum_check"], "l2": r["l2"], "clocks": r["clocks"], "occupancy": r["occupancy"],
     }
 
 
@@ -341,6 +361,7 @@ def main_b200(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "n": n, "cpd": cfg.cpd, "R": cfg.R, "eps": cfg.eps, "L": cfg.L,
                    "interactions_per_step": I, "l2": r["l2"], "multi_gpu": "replicas only (no collective)",
+                   "occupancy": r["occupancy"],
                    "flops_per_interaction": FLOPS_PER_INTERACTION},
         "particle_updates_per_s": world * n * K / (t_total / 1e3),
         "fp32_peak_frac": s["fp32_peak_frac_25flop"], "fp32_peak_frac_26flop_paper": s["fp32_peak_frac_26flop_paper"],

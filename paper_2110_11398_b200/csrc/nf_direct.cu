@@ -158,7 +158,11 @@ constexpr uint32_t kFull = 0xffffffffu;
 #ifndef NF_UNROLL_SOFT
 #define NF_UNROLL_SOFT 2
 #endif
-constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable piece loop
+constexpr int kUnrollSoft = NF_UNROLL_SOFT;
+#ifndef NF_UNROLL_TAIL
+#define NF_UNROLL_TAIL 8
+#endif
+constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)   // unrolling of the spline-capable piece loop
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
 
 // Newtonian part of two packed interactions: d, r^2, 1/r and k = r^-3
@@ -191,13 +195,13 @@ __device__ __forceinline__ void pair_density(const float2 r2, const SoftCoef &c,
     rho = __fadd2_rn(rho, w);
 }
 
-// Four sources against the sink of every lane.  With MODE >= 1 all 32 lanes must call it together (warp vote
-// inside): the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s -- a
+// Four sources against the sink of every lane.  With MODE >= 1 exactly the lanes of `mask` must call it together
+// (warp vote inside): the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s -- a
 // fraction of a percent of the quads at production density; otherwise the body is the Newtonian one plus
 // three FMNMX, a vote and a branch.
 template <bool PACKED, int MODE>
 __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float sxi, const float syi,
-                                     const float szi, const SoftCoef &c, Partial &f)
+                                     const float szi, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
 {
     if (PACKED && MODE == 0) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
@@ -209,7 +213,7 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
         pair_head(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c.tiny, dxa, dya, dza, r2a, ria, ka);
         pair_head(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c.tiny, dxb, dyb, dzb, r2b, rib, kb);
         const float m = fminf(fminf(r2a.x, r2a.y), fminf(r2b.x, r2b.y));
-        if (__any_sync(kFull, m < c.soft_r2)) {
+        if (__any_sync(mask, m < c.soft_r2)) {
             pair_spline(r2a, ria, c, ka);
             pair_spline(r2b, rib, c, kb);
         }
@@ -231,24 +235,29 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
     }
 }
 
-// One step of a warp: every lane runs over ITS piece (n4 quads at px); nmin / nmax are the warp's smallest and
-// largest n4.  The first loop is uniform; in the ragged tail a lane that has run out of sources is predicated
-// off (Newtonian body) or reads the stage's dummy quad (coordinates 2^55: contributes exactly 0 to the force
-// and to the density) so that the warp stays converged for the vote of the spline body.
+// One step of a warp: every lane runs over ITS piece (n4 quads at px).  `live` = lanes that have a piece in this
+// stage (n4 > 0), nmin / nmax = smallest / largest n4 among them.  The first loop is uniform over the live lanes;
+// in the ragged tail a lane that has run out of sources is predicated off (Newtonian body) or reads the stage's
+// dummy quad (coordinates 2^55: contributes exactly 0 to the force and to the density) so that the warp stays
+// converged for the vote of the spline body.
 template <bool PACKED, int MODE>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
-                                           const int jdummy, const float sxi, const float syi, const float szi,
+                                           const uint32_t live, const int jdummy, const float sxi, const float syi, const float szi,
                                            const SoftCoef &c, Partial &f)
 {
     const float4 *__restrict__ py = px + kTileAlloc / 4;
     const float4 *__restrict__ pz = py + kTileAlloc / 4;
-    if (MODE == 0) {
+    if (n4 > 0) {
+        if (MODE == 0) {
 #pragma unroll 2
-        for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
-    } else {
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+        } else {
 #pragma unroll kUnrollSoft
-        for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f, live);
+        }
     }
+    __syncwarp();
+#pragma unroll kUnrollTail
     for (int j = nmin; j < nmax; j++) {
         if (MODE >= 1 && PACKED) {                    // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
@@ -456,7 +465,8 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                 }
                 const int nmax = __reduce_max_sync(kFull, n4);
                 if (nmax == 0) continue;
-                const int nmin = __reduce_min_sync(kFull, n4);
+                const int nmin = __reduce_min_sync(kFull, n4 > 0 ? n4 : 0x7fffffff);   // over the lanes that have a piece
+                const uint32_t live = __ballot_sync(kFull, n4 > 0);
                 const float szi = (float)(czs - oczs) - zi;
                 const float4 *px = sbase + (sm_off >> 2);
                 const int jdummy = (kTile - sm_off) >> 2;           // the dummy quad, relative to px
@@ -468,9 +478,9 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                     if (soft_mode == 1) soft = __any_sync(kFull, gap2 < a.k.soft_thr2);
                     if (gap_dens) dens = __any_sync(kFull, gap2 < a.dens_thr2);
                 }
-                if (DENS && dens) piece_loop<PACKED, 2>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
-                else if (soft)    piece_loop<PACKED, 1>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
-                else              piece_loop<PACKED, 0>(px, n4, nmin, nmax, jdummy, sxi, syi, szi, coef, f);
+                if (DENS && dens) piece_loop<PACKED, 2>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                else if (soft)    piece_loop<PACKED, 1>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                else              piece_loop<PACKED, 0>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
             }
             ax += (double)f.x.x + (double)f.x.y;
             ay += (double)f.y.x + (double)f.y.y;
@@ -500,7 +510,8 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
 template <bool PACKED, bool DENS, bool EPI>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
-    __shared__ SharedStorage sm;
+    extern __shared__ __align__(128) unsigned char smem_raw[];          // dynamic: stages above 48 KB need the opt-in
+    SharedStorage &sm = *reinterpret_cast<SharedStorage *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < kStages * 3 * 4) sm.buf[tid / 12][(tid / 4) % 3][kTile + (tid & 3)] = kDummy;
     if (tid == 0) {
@@ -522,7 +533,9 @@ static direct_fn pick_kernel(int variant, bool dens, bool epi)      // dens and 
 int accel_max_ctas_per_sm(int variant)
 {
     int nb = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick_kernel(variant, false, false), kAccelThreads, 0);
+    direct_fn fn = pick_kernel(variant, false, false);
+    cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SharedStorage));
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, kAccelThreads, sizeof(SharedStorage));
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
@@ -538,7 +551,8 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     const bool dens = rho != nullptr;
     direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr);
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+    NF_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SharedStorage)));
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, sizeof(SharedStorage)) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
     if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
     if (p->ctas_per_sm > 0 && p->ctas_per_sm < per_sm) per_sm = p->ctas_per_sm;
     long long grid = (long long)p->sm_count * per_sm;
@@ -564,7 +578,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     NF_CUDA_OK(cudaEventRecord(p->ev[2], st));
     NF_CUDA_OK(cudaMemsetAsync(a.counter, 0, 4, st));
     if (amax_cell) NF_CUDA_OK(cudaMemsetAsync(amax_cell, 0, 4 * (size_t)p->k.ncells, st));
-    fn<<<(unsigned)grid, kAccelThreads, 0, st>>>(a);
+    fn<<<(unsigned)grid, kAccelThreads, sizeof(SharedStorage), st>>>(a);
     NF_CUDA_OK(cudaGetLastError());
     NF_CUDA_OK(cudaEventRecord(p->ev[3], st));
     p->have_accel_time = true;

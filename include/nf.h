@@ -25,6 +25,9 @@
  * pointers (pinned memory makes the copies asynchronous).  The library never frees or keeps caller
  * memory past the call unless stated.  No torch types cross this boundary.
  *
+ * A plan belongs to the CUDA device that is current at its first nf_bin; later calls switch to that device for
+ * their duration if another one is current.
+ *
  * Return values: 0 = NF_OK, negative = error; nf_last_error() gives a thread-local message.
  * There is NO CPU fallback: without a CUDA device every compute call fails with NF_ERR_CUDA.
  */

@@ -125,6 +125,19 @@ static int ensure_stage(nf_plan *p, long long n)
     return NF_OK;
 }
 
+// A plan lives on the device that was current at its first nf_bin; later calls made while another device is current
+// switch to it for the duration of the call.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const nf_plan *p)
+    {
+        int cur = -1;
+        if (p && p->device >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != p->device && cudaSetDevice(p->device) == cudaSuccess)
+            prev = cur;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 // Softening constants of the pair bodies.  kind 0: the compact spline (readings C2/C3); kind 1: Plummer.
 static int set_softening(nf_plan *p, int kind)
 {
@@ -246,7 +259,8 @@ int nf_set_sink_slabs(nf_plan *p, int x_first, int n_slabs)
 }
 
 int nf_bin(nf_plan *p, const float *pos, long long n)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     p->binned = false;
     if (n < 0) { set_error("n < 0"); return NF_ERR_ARG; }
@@ -263,7 +277,8 @@ int nf_bin(nf_plan *p, const float *pos, long long n)
 }
 
 int nf_accel(nf_plan *p, float *acc)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel called before a successful nf_bin"); return NF_ERR_STATE; }
     if (!acc && p->n > 0) { set_error("null acc"); return NF_ERR_ARG; }
@@ -271,7 +286,8 @@ int nf_accel(nf_plan *p, float *acc)
 }
 
 int nf_accel_density(nf_plan *p, float *acc, float *rho, double b)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel_density called before a successful nf_bin"); return NF_ERR_STATE; }
     if ((!acc || !rho) && p->n > 0) { set_error("null acc or rho"); return NF_ERR_ARG; }
@@ -285,7 +301,8 @@ int nf_accel_density(nf_plan *p, float *acc, float *rho, double b)
 }
 
 int nf_accel_kick(nf_plan *p, float *acc, float *vel, double dt, float *amax_cell)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel_kick called before a successful nf_bin"); return NF_ERR_STATE; }
     if (!acc && !vel && !amax_cell) { set_error("nf_accel_kick: acc, vel and amax_cell are all null"); return NF_ERR_ARG; }
@@ -298,7 +315,8 @@ int nf_accel_kick(nf_plan *p, float *acc, float *vel, double dt, float *amax_cel
 }
 
 int nf_bin_host(nf_plan *p, const float *pos_host, long long n)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     p->binned = false;
     if (n < 0 || (!pos_host && n > 0)) { set_error("bad pos_host / n"); return NF_ERR_ARG; }
@@ -311,7 +329,8 @@ int nf_bin_host(nf_plan *p, const float *pos_host, long long n)
 }
 
 int nf_accel_host(nf_plan *p, float *acc_host)
-{
+{    DeviceGuard guard(p);
+
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     if (!p->binned) { set_error("nf_accel_host called before a successful nf_bin"); return NF_ERR_STATE; }
     if (!acc_host && p->n > 0) { set_error("null acc_host"); return NF_ERR_ARG; }
@@ -352,7 +371,8 @@ int nf_get_layout(const nf_plan *p, const unsigned **poff, const float **x, cons
 }
 
 int nf_get_stats(nf_plan *p, nf_stats *out)
-{
+{    DeviceGuard guard(p);
+
     if (!p || !out) { set_error("null argument"); return NF_ERR_ARG; }
     memset(out, 0, sizeof(*out));
     out->cells = p->k.ncells;

@@ -103,7 +103,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
-struct SoftCoef { float A, B, C, tiny, soft_r2, nb2; int plummer; };   // nb2 = -1/b^2 of the density kernel
+struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin)
 
 // two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
 // (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ
@@ -217,7 +217,7 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
             pair_spline(r2a, ria, c, ka);
             pair_spline(r2b, rib, c, kb);
         }
-        if (MODE == 2) {
+        if (MODE == 2 && __any_sync(mask, m < c.dens_r2)) {     // some lane has a source of this quad inside b
             if (c.plummer) {                  // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
                 r2a = __ffma2_rn(dxa, dxa, __ffma2_rn(dya, dya, __fmul2_rn(dza, dza)));
                 r2b = __ffma2_rn(dxb, dxb, __ffma2_rn(dyb, dyb, __fmul2_rn(dzb, dzb)));
@@ -400,7 +400,8 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
 template <bool PACKED, bool DENS, bool EPI>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
 {
-    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f, a.k.plummer};
+    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f,
+                           DENS ? -1.001f / a.dens_nb2 + a.k.tiny : 0.f, a.k.plummer};
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;

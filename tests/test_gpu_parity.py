@@ -567,3 +567,36 @@ def test_bitwise_determinism():
             outs.append((a1, a2.clone(), rho.clone()))
     for o in outs[1:]:
         assert all(torch.equal(x, y) for x, y in zip(o, outs[0]))
+
+
+def test_config4_full_size_density_and_kick_sampled(oracle_mod):
+    """The fused passes at the clustered production size (cells of 2.6e5 particles): density, kick and per-cell maxima on
+    the sink sample, accelerations of the fused passes bit-identical to nf_accel."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.config(4)
+    pos_dev = nf_inputs.generate(cfg, device="cuda")
+    pos = pos_dev.cpu().numpy()
+    b = oracle_mod.bin_particles(pos, cfg.cpd, cfg.L)
+    sinks = sample_sinks(b["count"], b["offset"], b["perm"], cfg.cpd, np.random.default_rng(44), n_random=500, n_heavy=10, per_heavy=100)
+    bw = 0.4 * cfg.L / cfg.n_side
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos_dev)
+        acc = plan.accel()
+        acc_d, rho = plan.accel_density(bw)
+        vel = torch.zeros_like(pos_dev)
+        acc_k, amax = plan.accel_kick(vel, 2.0 ** -20)
+        torch.cuda.synchronize()
+    assert torch.equal(acc_k, acc) and torch.equal(vel, acc * 2.0 ** -20)
+    assert (acc_d - acc).norm().item() <= 1e-6 * acc.norm().item()
+    idx = torch.from_numpy(sinks).cuda()
+    ref_rho = oracle_mod.density(pos, cfg.cpd, cfg.L, bw, cfg.R, sinks=sinks, binning=b)
+    err = np.abs(rho[idx].cpu().numpy().astype(np.float64) - ref_rho) / ref_rho
+    assert err.max() <= TOL_RHO, err.max()
+    ref = oracle_mod.accel(pos, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=sinks, binning=b)
+    st = assert_parity(acc[idx].cpu().numpy().astype(np.float64), ref, cfg.name + " fused passes (sampled)")
+    # per-cell maxima: exact maximum of the float32 norms the kernel wrote, for every cell
+    norms = acc.double().norm(dim=1)
+    cid = torch.from_numpy(b["cid"].astype(np.int64)).cuda()
+    m_ref = torch.zeros(cfg.cpd ** 3, dtype=torch.float64, device="cuda").scatter_reduce_(0, cid, norms, "amax")
+    assert torch.allclose(amax.double(), m_ref, rtol=2e-7, atol=0)
+    print(cfg.name, "fused passes", st, "rho max err", float(err.max()), "rho max", float(ref_rho.max()))

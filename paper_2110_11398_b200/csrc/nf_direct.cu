@@ -407,7 +407,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
     uint32_t phase = 0;
     float xi = 0.f, yi = 0.f, zi = 0.f;
     double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0, rho = 0.0;
-    int zrel = 0;                       // the lane's sink cell, relative to z0
+    int zrel = 0, zoff = 0;             // the lane's sink cell relative to z0, and zrel mod (2R+1)
     uint32_t slot = 0;                  // the lane's sorted slot (perm index)
     uint32_t cell = 0;                  // the lane's sink cell id
     bool act = false, warp_on = false;
@@ -431,6 +431,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                     if (__ldg(off + mid) <= slot) lo = mid; else hi = mid - 1;
                 }
                 zrel = lo - (int)d.z0;
+                zoff = zrel % nsteps;
                 if (EPI) cell = d.colbase + (uint32_t)lo;
                 const uint32_t p = __ldg(a.poff + d.colbase + lo) + (slot - __ldg(off + lo));
                 xi = __ldg(a.x + p); yi = __ldg(a.y + p); zi = __ldg(a.z + p);
@@ -455,7 +456,13 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
             const float4 *sbase = reinterpret_cast<const float4 *>(&sm.buf[stage][0][0]);
             Partial f;
             f.clear();
-            for (int t = 0; t < nsteps; t++) {
+            // Step s pairs the lanes of the warp by SOURCE cell: a lane takes the one cell j of its stencil with
+            // (j - (z0 - R)) mod (2R+1) == s.  Lanes of different sink cells then read the same piece in all steps but
+            // the few where the stencils do not overlap (cells j and j + 2R+1 share a step), so the piece lengths of
+            // a step differ between lanes only there.
+            for (int s = 0; s < nsteps; s++) {
+                int t = s - zoff;                                   // offset of that cell from zc - R, in [0, 2R]
+                t += t < 0 ? nsteps : 0;
                 const int idx = ibase + t;                          // the lane's piece for cell zc - R + t
                 const bool valid = (unsigned)idx < (unsigned)np;
                 int n4 = 0, sm_off = 0;
@@ -473,11 +480,12 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                 const int jdummy = (kTile - sm_off) >> 2;           // the dummy quad, relative to px
                 const int dt = t - R;
                 bool soft = soft_mode == 2, dens = DENS && a.dens_mode == 2;
-                if ((soft_mode == 1 || gap_dens) && dt >= -1 && dt <= 1) {
+                if (soft_mode == 1 || gap_dens) {                   // warp-uniform; dt is per lane
+                    const bool touching = n4 > 0 && dt >= -1 && dt <= 1;
                     const float gz = dt < 0 ? zi : (dt > 0 ? a.k.w_scaled - zi : 0.f);
                     const float gap2 = fmaf(gz, gz, gxy2);
-                    if (soft_mode == 1) soft = __any_sync(kFull, gap2 < a.k.soft_thr2);
-                    if (gap_dens) dens = __any_sync(kFull, gap2 < a.dens_thr2);
+                    if (soft_mode == 1) soft = __any_sync(kFull, touching && gap2 < a.k.soft_thr2);
+                    if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
                 if (DENS && dens) piece_loop<PACKED, 2>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
                 else if (soft)    piece_loop<PACKED, 1>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);

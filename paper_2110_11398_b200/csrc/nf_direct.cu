@@ -13,10 +13,10 @@
 //   * for each of the (2R+1)^2 neighbour columns the producer streams the z-run of cells [z0-R, z1+R] that the
 //     window's sinks need into shared memory with TMA 1-D bulk copies (cp.async.bulk + mbarrier complete_tx)
 //     through a kStages-deep ring, with a table of the cells (pieces) of the run;
-//   * a lane whose sink sits in cell zc walks ITS OWN 2R+1 pieces zc-R..zc+R of the run: in step t every
-//     lane of the warp reads the piece at offset t-R from its own cell, so lanes of different cells read
-//     different pieces in the same instruction (per-lane shared-memory pointer, one LDS.128 wavefront per
-//     distinct cell) and no lane ever evaluates a pair outside its stencil;
+//   * a lane whose sink sits in cell zc walks ITS OWN 2R+1 pieces zc-R..zc+R of the run (per-lane shared-memory
+//     pointer), so no lane ever evaluates a pair outside its stencil; the order pairs the lanes of a warp by
+//     source cell (step s takes the cell j with (j - z0 + R) mod (2R+1) == s), so lanes of neighbouring sink
+//     cells read the same piece except in the one step where their stencils do not overlap;
 //   * one sink per lane in registers; sources are read as LDS.128 of 4 x, 4 y, 4 z and processed as two
 //     packed pairs with FFMA2/FADD2/FMUL2 (fma.rn.f32x2), one MUFU.RSQ per interaction;
 //   * coordinates are cell-corner relative (exact); the periodic wrap and the cell-to-cell shift are one

@@ -348,6 +348,60 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
                     uint32_t P0 = 0, P1 = 0;
                     if (jl <= jhi) { P0 = __ldg(a.poff + row + jwl); P1 = __ldg(a.poff + row + jwl + 1); }
                     const int cnt = min(32, jhi - jb + 1);
+                    // Fast path (all lanes in parallel): when the whole chunk of <= 32 cells fits the open stage, or a
+                    // fresh one, every lane writes the table entry of its cell and lane 0 issues one merged copy per
+                    // contiguous segment (a segment ends at the periodic z face).  Sparse regions, where a window of
+                    // sinks spans dozens of cells, would otherwise serialise on the per-cell loop below.
+                    {
+                        const uint32_t nsl = lane < cnt ? P1 - P0 : 0u;
+                        uint32_t inc = nsl;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const uint32_t up = __shfl_up_sync(kFull, inc, o);
+                            if (lane >= o) inc += up;
+                        }
+                        const uint32_t total = __shfl_sync(kFull, inc, 31);
+                        const uint32_t off = inc - nsl;
+                        if (total == 0 && (!open || sealed)) continue;          // empty cells never open a stage
+                        const bool can_append = open && !sealed && fill + (int)total <= kTile && np + cnt <= kMaxPieces;
+                        const bool can_open = (int)total <= kTile && cnt <= kMaxPieces;
+                        if (can_append || can_open) {
+                            if (!can_append) {
+                                if (open) commit(0);
+                                mbar_wait(&sm.empty[stage], phase ^ 1u);
+                                open = true; fill = 0; np = 0;
+                                sflags = first ? kFlagBegin : 0;
+                                first = false;
+                                if (lead) {
+                                    StageDesc &d = sm.desc[stage];
+                                    d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 8) | ((oy + 8) << 8);
+                                    d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.colbase = un.col * (uint32_t)cpd;
+                                }
+                            }
+                            if (lane < cnt) {
+                                const double wz = jl < 0 ? -k.L : (jl >= cpd ? k.L : 0.0);
+                                Piece &pc = sm.desc[stage].pieces[np + lane];
+                                pc.sm_off = fill + (int)off; pc.nslots = (int)nsl;
+                                pc.czs = ((double)(float)((double)jwl * k.cell_w) + wz) * k.scale;
+                            }
+                            uint32_t starts = __ballot_sync(kFull, lane < cnt && (lane == 0 || jwl == 0));
+                            while (starts) {
+                                const int b = __ffs(starts) - 1;
+                                starts &= starts - 1;
+                                const int e = starts ? __ffs(starts) - 1 : cnt;     // segment = lanes [b, e)
+                                const uint32_t g0 = __shfl_sync(kFull, P0, b);
+                                const uint32_t o0 = __shfl_sync(kFull, off, b);
+                                const uint32_t len = __shfl_sync(kFull, inc, e - 1) - o0;
+                                if (len == 0) continue;
+                                const uint32_t s0 = (uint32_t)fill + o0;
+                                if (cp_n && cp_g + cp_n == g0 && cp_s + cp_n == s0) cp_n += len;
+                                else { flush_copy(); cp_g = g0; cp_s = s0; cp_n = len; }
+                            }
+                            np += cnt; fill += (int)total;
+                            continue;
+                        }
+                    }
                     for (int q = 0; q < cnt; q++) {
                         uint32_t p0 = __shfl_sync(kFull, P0, q);
                         const uint32_t p1 = __shfl_sync(kFull, P1, q);

@@ -28,7 +28,7 @@ constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // sink lanes per CTA = 32 * k
 constexpr int kChunk         = 32 * kConsumerWarps;   // max sinks per work unit (a window of one z-column)
 constexpr int kTile          = NF_TILE;           // source slots per pipeline stage (multiple of 4)
 constexpr int kStages        = NF_STAGES;         // TMA pipeline depth
-constexpr int kMaxPieces     = 24;                // source cells (table entries) per stage
+constexpr int kMaxPieces     = 40;                // source cells (table entries) per stage
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
 constexpr int kMinCtasPerSm  = NF_MIN_CTAS;       // register budget: 65536 / (kMinCtasPerSm * kAccelThreads) per thread
 #ifndef NF_WAIT_SLEEP_NS

@@ -26,7 +26,7 @@ UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
 FLOPS_EXECUTED_MIN = 19         # the Newtonian body (3 add + 6 fma + 2 mul + rsqrt) the kernel runs where no pair is inside eps_s
 # DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v5_direct_kernel.md)
-NCU_TRAFFIC_BYTES = {"config3_uniform_256": 961722368 + 657881856, "config4_halos_512": 18111688000 + 5377143000}
+NCU_TRAFFIC_BYTES = {"config3_uniform_256": 961545472 + 659134976, "config4_halos_512": 18111688000 + 5377143000}
 L2_BYTES = 126 * 1024 * 1024
 
 

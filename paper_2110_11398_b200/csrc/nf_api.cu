@@ -39,14 +39,18 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     const size_t ncol = (size_t)cpd * cpd;
     const size_t umax = (N < ncol ? N : ncol) + N / kChunk + 2;    // every column ends with one ragged window
     const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
-    const size_t sort_blocks = (nsort + kSortTile - 1) / kSortTile + 1;
-    const size_t scan_items = (256 * sort_blocks > C + 2 ? 256 * sort_blocks : C + 2);
+    int sort_passes = 1, sort_bits = kSortMinBits;
+    sort_plan((unsigned long long)C, &sort_passes, &sort_bits);
+    const size_t hist_particles = ((size_t)1 << sort_bits) * ((N + kSortTile - 1) / kSortTile + 1);
+    const size_t hist_units = ((size_t)1 << kSortMinBits) * ((umax + kSortTile - 1) / kSortTile + 1);
+    const size_t hist_items = hist_particles > hist_units ? hist_particles : hist_units;
+    const size_t scan_items = (hist_items > C + 2 ? hist_items : C + 2);
     ws.cid  = (uint32_t *)take(4 * (N + 1));
     ws.keyA = (uint32_t *)take(4 * nsort);
     ws.keyB = (uint32_t *)take(4 * nsort);
     ws.valA = (uint32_t *)take(4 * nsort);
     ws.valB = (uint32_t *)take(4 * nsort);
-    ws.radix_hist = (uint32_t *)take(4 * 256 * sort_blocks);
+    ws.radix_hist = (uint32_t *)take(4 * hist_items);
     ws.count  = (uint32_t *)take(4 * (C + 1));
     ws.offset = (uint32_t *)take(4 * (C + 2));
     ws.poff   = (uint32_t *)take(4 * (C + 2));

@@ -113,131 +113,303 @@ static void exclusive_scan(const uint32_t *in, uint32_t *out, size_t n, uint32_t
     *launches += 3;
 }
 
-// ---- S1 + S2: cell id (float64 index formula, reading C6) and histogram ---------------------------
-__global__ void __launch_bounds__(256) cellid_kernel(const float *__restrict__ pos, size_t n, Consts k,
-                                                     uint32_t *__restrict__ cid, uint32_t *__restrict__ count,
-                                                     uint32_t *__restrict__ scalars)
+// ---- S1 + S2: cell id (float64 index formula, reading C6), per-cell histogram, digit histogram of the first sort pass
+// One block per sort tile (kSortTile particles), so that the block's digit counts are the column of the first
+// pass's histogram matrix and the ids are not read again for it.
+__global__ void __launch_bounds__(kSortThreads) cellid_kernel(const float *__restrict__ pos, size_t n, Consts k,
+                                                              uint32_t *__restrict__ cid, uint32_t *__restrict__ count,
+                                                              uint32_t *__restrict__ scalars, uint32_t digit_mask,
+                                                              uint32_t *__restrict__ hist, uint32_t nblocks)
 {
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float *p = pos + 3 * i;
-    int c[3];
-    bool bad = false;
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
-        double x = (double)p[d];
-        if (!(x >= 0.0 && x < k.L)) bad = true;        // also catches NaN; +-inf
-        int q = (int)floor(x * k.inv_cell_w);
-        q = q >= k.cpd ? k.cpd - 1 : (q < 0 ? 0 : q);
-        c[d] = q;
-    }
-    uint32_t id = ((uint32_t)c[0] * k.cpd + c[1]) * k.cpd + c[2];
-    cid[i] = id;
-    if (bad) atomicOr(&scalars[0], 1u);
-    atomicAdd(&count[id], 1u);
-}
-
-// ---- S4: stable LSD radix sort of (cell id, input index), 8 bits per pass ------------------------------
-__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const uint32_t *__restrict__ kin, size_t n, int shift,
-                                                                  uint32_t *__restrict__ hist, uint32_t nblocks)
-{
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
+    __shared__ uint32_t h[1 << kSortMaxBits];
+    for (uint32_t d = threadIdx.x; d <= digit_mask; d += kSortThreads) h[d] = 0;
     __syncthreads();
-    size_t base = (size_t)blockIdx.x * kSortTile;
+    const size_t base = (size_t)blockIdx.x * kSortTile;
+    bool bad = false;
 #pragma unroll 4
     for (int r = 0; r < kSortItems; r++) {
-        size_t e = base + (size_t)r * kSortThreads + threadIdx.x;
-        if (e < n) atomicAdd(&h[(kin[e] >> shift) & 255u], 1u);
+        const size_t i = base + (size_t)r * kSortThreads + threadIdx.x;
+        if (i >= n) break;
+        const float *p = pos + 3 * i;
+        int c[3];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            double x = (double)p[d];
+            if (!(x >= 0.0 && x < k.L)) bad = true;        // also catches NaN; +-inf
+            int q = (int)floor(x * k.inv_cell_w);
+            q = q >= k.cpd ? k.cpd - 1 : (q < 0 ? 0 : q);
+            c[d] = q;
+        }
+        const uint32_t id = ((uint32_t)c[0] * k.cpd + c[1]) * k.cpd + c[2];
+        cid[i] = id;
+        atomicAdd(&count[id], 1u);
+        atomicAdd(&h[id & digit_mask], 1u);
     }
+    if (bad) atomicOr(&scalars[0], 1u);
     __syncthreads();
-    hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+    for (uint32_t d = threadIdx.x; d <= digit_mask; d += kSortThreads) hist[(size_t)d * nblocks + blockIdx.x] = h[d];
 }
 
-// Each warp owns a contiguous 512-key segment of the block's tile and ranks it in input order with
-// match_any, so the scatter is stable: equal digits keep ascending input position (reading C9).
-template <bool IOTA>
-__global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(const uint32_t *__restrict__ kin, const uint32_t *__restrict__ vin,
-                                                                     uint32_t *__restrict__ kout, uint32_t *__restrict__ vout,
-                                                                     size_t n, int shift, const uint32_t *__restrict__ hist,
-                                                                     uint32_t nblocks)
+// ---- S4: stable LSD radix sort of (cell id, input index), 8-11 bits per pass, gather fused into the last pass -------
+__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const uint32_t *__restrict__ kin, size_t n, int shift,
+                                                                  uint32_t digit_mask, uint32_t *__restrict__ hist,
+                                                                  uint32_t nblocks)
 {
-    __shared__ uint32_t cnt[kSortWarps][256];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int q = threadIdx.x; q < kSortWarps * 256; q += kSortThreads) (&cnt[0][0])[q] = 0;
+    __shared__ uint32_t h[1 << kSortMaxBits];
+    for (uint32_t d = threadIdx.x; d <= digit_mask; d += kSortThreads) h[d] = 0;
     __syncthreads();
-    const size_t seg = (size_t)blockIdx.x * kSortTile + (size_t)w * (32 * kSortItems);
-    uint32_t key[kSortItems], lr[kSortItems];
-    const uint32_t lt = (1u << lane) - 1u;
+    const size_t base = (size_t)blockIdx.x * kSortTile;
+#pragma unroll 4
+    for (int r = 0; r < kSortItems; r++) {
+        const size_t e = base + (size_t)r * kSortThreads + threadIdx.x;
+        if (e < n) atomicAdd(&h[(kin[e] >> shift) & digit_mask], 1u);
+    }
+    __syncthreads();
+    for (uint32_t d = threadIdx.x; d <= digit_mask; d += kSortThreads) hist[(size_t)d * nblocks + blockIdx.x] = h[d];
+}
+
+// What the last pass needs to write the cell-padded SoA source arrays instead of sorted keys (S4, second half):
+// values are (pos - corner(cell)) * 2^k; both steps are exact in float32 (Sterbenz), see the file header.
+struct GatherArgs {
+    const float *pos;
+    const uint32_t *offset, *poff;
+    float *X, *Y, *Z;
+    Consts k;
+};
+
+// One pass.  Each warp owns a contiguous 512-key segment of the block's tile and ranks it in input order with
+// match_any, so the pass is stable: equal digits keep ascending input position (reading C9).  The tile is then put
+// in digit order in shared memory so that consecutive threads write consecutive destinations.
+//   IOTA: the values are the positions themselves (first pass);
+//   LAST: the keys are whole cell ids in their final order: write perm and the padded SoA arrays, no keys.
+// Lanes of the warp that hold the same BITS-bit digit as the caller (only valid lanes are counted; the result of an
+// invalid lane is unused).  One ballot per bit: MATCH.ANY takes time in proportion to the number of distinct values
+// in the warp, which for 9-11 bit digits of unsorted keys is nearly 32 (measured: half of the stall samples of a pass).
+template <int BITS>
+__device__ __forceinline__ uint32_t match_digit(const uint32_t d, const bool valid)
+{
+    uint32_t m = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+    for (int b = 0; b < BITS; b++) {
+        const uint32_t bit = (d >> b) & 1u;
+        m &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
+    }
+    return m;
+}
+
+constexpr int kRankBatch = 4;      // rounds of the ranking whose shared-memory atomics are in flight together
+
+template <int BITS, bool IOTA, bool LAST>
+__global__ void __launch_bounds__(kSortThreads, 2) radix_scatter_kernel(const uint32_t *__restrict__ kin, const uint32_t *__restrict__ vin,
+                                                                        uint32_t *__restrict__ kout, uint32_t *__restrict__ vout,
+                                                                        size_t n, int shift, const uint32_t *__restrict__ hist,
+                                                                        uint32_t nblocks, const GatherArgs g)
+{
+    constexpr int BINS = 1 << BITS;
+    constexpr uint32_t MASK = BINS - 1;
+    constexpr int DPT = BINS >= kSortThreads ? BINS / kSortThreads : 1;        // digits per thread in the scans
+    extern __shared__ __align__(16) unsigned char sort_smem[];
+    // [0, 64 KB): per-warp digit counters during ranking, then the reordered tile (keys, values)
+    uint16_t (*cnt)[BINS] = reinterpret_cast<uint16_t (*)[BINS]>(sort_smem);
+    uint32_t *skey = reinterpret_cast<uint32_t *>(sort_smem);
+    uint32_t *sval = skey + kSortTile;
+    uint32_t *lbase = sval + kSortTile;                    // first tile-local position of each digit
+    uint32_t *gdelta = lbase + BINS;                       // global destination of the digit's first key - lbase
+    uint32_t *scan_sm = gdelta + BINS;                     // [33]
+
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    {
+        uint32_t *z = reinterpret_cast<uint32_t *>(sort_smem);
+        for (int q = threadIdx.x; q < kSortWarps * BINS / 2; q += kSortThreads) z[q] = 0;
+    }
+    const size_t tile0 = (size_t)blockIdx.x * kSortTile;
+    const size_t seg = tile0 + (size_t)w * (32 * kSortItems);
+    uint32_t key[kSortItems], lr[kSortItems / 2];     // ranks / tile-local positions: two 16-bit values per register
+#pragma unroll
+    for (int r = 0; r < kSortItems / 2; r++) lr[r] = 0;
 #pragma unroll
     for (int r = 0; r < kSortItems; r++) {
-        size_t e = seg + r * 32 + lane;
-        bool valid = e < n;
-        key[r] = valid ? kin[e] : 0u;
-        uint32_t d = (key[r] >> shift) & 255u;
-        uint32_t mask = __match_any_sync(0xffffffffu, valid ? d : (256u + lane));
-        uint32_t old = valid ? cnt[w][d] : 0u;
-        __syncwarp();
-        if (valid && lane == __ffs(mask) - 1) cnt[w][d] = old + __popc(mask);
-        __syncwarp();
-        lr[r] = old + __popc(mask & lt);
+        const size_t e = seg + r * 32 + lane;
+        key[r] = e < n ? kin[e] : 0u;
+    }
+    __syncthreads();
+    // Rank of a key among the keys of its digit in the warp's segment: the lanes holding the digit are found with
+    // match_any, the first of them adds their number to the warp's counter of the digit (two 16-bit counters per word;
+    // a segment has 512 keys) and hands the old value to the others.  The rounds depend on each other only through
+    // the order of the shared-memory atomics of the warp, so their latencies overlap.
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t *cw = reinterpret_cast<uint32_t *>(sort_smem) + w * (BINS / 2);
+#pragma unroll
+    for (int h = 0; h < kSortItems; h += kRankBatch) {
+        uint32_t m[kRankBatch], o[kRankBatch];
+#pragma unroll
+        for (int r = 0; r < kRankBatch; r++) {
+            const bool valid = seg + (h + r) * 32 + lane < n;
+            const uint32_t d = (key[h + r] >> shift) & MASK;
+            m[r] = match_digit<BITS>(d, valid);
+        }
+#pragma unroll
+        for (int r = 0; r < kRankBatch; r++) {
+            const bool valid = seg + (h + r) * 32 + lane < n;
+            const uint32_t d = (key[h + r] >> shift) & MASK;
+            o[r] = 0;
+            if (valid && (m[r] & lt) == 0) o[r] = atomicAdd(&cw[d >> 1], (uint32_t)__popc(m[r]) << ((d & 1u) * 16));
+        }
+#pragma unroll
+        for (int r = 0; r < kRankBatch; r++) {
+            const uint32_t d = (key[h + r] >> shift) & MASK;
+            const uint32_t old = (__shfl_sync(0xffffffffu, o[r], __ffs(m[r]) - 1) >> ((d & 1u) * 16)) & 0xffffu;
+            lr[(h + r) >> 1] |= (old + __popc(m[r] & lt)) << (((h + r) & 1) * 16);
+        }
     }
     __syncthreads();
     {
-        const int d = threadIdx.x;                               // one digit per thread
-        uint32_t run = hist[(size_t)d * nblocks + blockIdx.x];
+        // per digit: exclusive scan over the warps; then the block-wide exclusive scan of the digit totals
+        const int d0 = threadIdx.x * DPT;
+        uint32_t tot[DPT], s = 0;
 #pragma unroll
-        for (int ww = 0; ww < kSortWarps; ww++) { uint32_t c = cnt[ww][d]; cnt[ww][d] = run; run += c; }
+        for (int q = 0; q < DPT; q++) {
+            uint32_t run = 0;
+            if (d0 + q < BINS) {
+#pragma unroll
+                for (int ww = 0; ww < kSortWarps; ww++) { const uint32_t c = cnt[ww][d0 + q]; cnt[ww][d0 + q] = (uint16_t)run; run += c; }
+            }
+            tot[q] = run; s += run;
+        }
+        uint32_t ex = block_exclusive_scan(s, nullptr, scan_sm);
+#pragma unroll
+        for (int q = 0; q < DPT; q++) {
+            if (d0 + q < BINS) {
+                lbase[d0 + q] = ex;
+                gdelta[d0 + q] = hist[(size_t)(d0 + q) * nblocks + blockIdx.x] - ex;
+                ex += tot[q];
+            }
+        }
     }
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < kSortItems; r++) {
-        size_t e = seg + r * 32 + lane;
-        if (e < n) {
-            uint32_t d = (key[r] >> shift) & 255u;
-            uint32_t dst = cnt[w][d] + lr[r];
-            kout[dst] = key[r];
-            vout[dst] = IOTA ? (uint32_t)e : vin[e];
+        const uint32_t d = (key[r] >> shift) & MASK;
+        lr[r >> 1] += (lbase[d] + cnt[w][d]) << ((r & 1) * 16);     // tile-local position in digit order (< 8192)
+    }
+    __syncthreads();                                       // the counters are dead: their storage takes the tile
+#pragma unroll
+    for (int r = 0; r < kSortItems; r++) {
+        const size_t e = seg + r * 32 + lane;
+        const uint32_t lp = (lr[r >> 1] >> ((r & 1) * 16)) & 0xffffu;
+        if (e < n) { skey[lp] = key[r]; sval[lp] = IOTA ? (uint32_t)e : vin[e]; }
+    }
+    __syncthreads();
+    const uint32_t tile_n = (uint32_t)(n - tile0 < (size_t)kSortTile ? n - tile0 : (size_t)kSortTile);
+    if (!LAST) {
+#pragma unroll 4
+        for (int r = 0; r < kSortItems; r++) {
+            const uint32_t i = r * kSortThreads + threadIdx.x;
+            if (i < tile_n) {
+                const uint32_t c = skey[i];
+                const uint32_t dst = gdelta[(c >> shift) & MASK] + i;
+                kout[dst] = c;
+                vout[dst] = sval[i];
+            }
+        }
+    } else {
+        // The 12 bytes of a particle sit anywhere in the input: the 96 floats of 32 consecutive sorted particles are
+        // fetched by the warp as 3 loads in which adjacent lanes read adjacent floats of one particle (a request touches
+        // ~14 sectors instead of 32) and handed to the owning lanes through shared memory.
+        float *xyz = reinterpret_cast<float *>(scan_sm + 40) + w * 96;
+        const Consts &k = g.k;
+        const float sc = (float)k.scale;
+        auto fetch = [&](int r, float (&f)[3]) {                       // the warp's loads of round r
+            const uint32_t i0 = r * kSortThreads + w * 32;
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                const uint32_t flat = j * 32 + lane, q = flat / 3u, comp = flat - 3u * q;
+                f[j] = (r < kSortItems && i0 + q < tile_n) ? __ldg(g.pos + 3 * (size_t)sval[i0 + q] + comp) : 0.f;
+            }
+        };
+        float fa[3], fb[3];
+        fetch(0, fa);
+        fetch(1, fb);
+        for (int r = 0; r < kSortItems; r++) {
+            const uint32_t i0 = r * kSortThreads + w * 32;           // warp-uniform
+            if (i0 >= tile_n) break;
+            const uint32_t i = i0 + lane;
+            const bool valid = i < tile_n;
+            const uint32_t c = valid ? skey[i] : 0u, v = valid ? sval[i] : 0u;
+#pragma unroll
+            for (int j = 0; j < 3; j++) { xyz[j * 32 + lane] = fa[j]; fa[j] = fb[j]; }
+            fetch(r + 2, fb);                                        // two rounds of loads stay in flight
+            __syncwarp();
+            if (valid) {
+                const uint32_t dst = gdelta[(c >> shift) & MASK] + i;
+                vout[dst] = v;
+                const uint32_t cz = c % k.cpd, cy = (c / k.cpd) % k.cpd, cx = c / (k.cpd * k.cpd);
+                // corner origins are float32 values; pos - origin is exact (Sterbenz), the power-of-two scale too
+                const float ox = (float)((double)cx * k.cell_w), oy = (float)((double)cy * k.cell_w), oz = (float)((double)cz * k.cell_w);
+                const uint32_t o0 = g.offset[c], o1 = g.offset[c + 1];
+                const uint32_t p = g.poff[c] + (dst - o0);
+                g.X[p] = (xyz[3 * lane + 0] - ox) * sc;
+                g.Y[p] = (xyz[3 * lane + 1] - oy) * sc;
+                g.Z[p] = (xyz[3 * lane + 2] - oz) * sc;
+                if (dst + 1 == o1) {
+                    const uint32_t pe = g.poff[c + 1];
+                    for (uint32_t q = p + 1; q < pe; q++) { g.X[q] = kDummy; g.Y[q] = kDummy; g.Z[q] = kDummy; }
+                }
+            }
+            __syncwarp();
         }
     }
 }
 
-// one pass; returns launches
-static void radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift,
-                       bool iota, uint32_t *hist, uint32_t *scan_tmp, cudaStream_t st, int *launches)
+template <int BITS>
+static size_t scatter_smem_bytes() { return 8 * (size_t)kSortTile + 8 * ((size_t)1 << BITS) + 4 * 40 + 4 * 96 * kSortWarps; }
+
+template <int BITS, bool IOTA, bool LAST>
+static cudaError_t scatter_launch(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift,
+                                  const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st)
 {
-    uint32_t nb = (uint32_t)((n + kSortTile - 1) / kSortTile);
-    radix_hist_kernel<<<nb, kSortThreads, 0, st>>>(kin, n, shift, hist, nb);
-    *launches += 1;
-    exclusive_scan(hist, hist, (size_t)256 * nb, scan_tmp, OpId(), 0, nullptr, st, launches);
-    if (iota) radix_scatter_kernel<true><<<nb, kSortThreads, 0, st>>>(kin, vin, kout, vout, n, shift, hist, nb);
-    else      radix_scatter_kernel<false><<<nb, kSortThreads, 0, st>>>(kin, vin, kout, vout, n, shift, hist, nb);
-    *launches += 1;
+    static_assert(2 * kSortWarps * (1 << BITS) <= 8 * kSortTile, "the counters must fit the tile storage");
+    auto fn = radix_scatter_kernel<BITS, IOTA, LAST>;
+    const size_t smem = scatter_smem_bytes<BITS>();
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    fn<<<nb, kSortThreads, smem, st>>>(kin, vin, kout, vout, n, shift, hist, nb, g);
+    return cudaGetLastError();
 }
 
-// ---- S4 (second half): gather into the padded, cell-relative, scaled SoA arrays -------------------------
-__global__ void __launch_bounds__(256) gather_kernel(const float *__restrict__ pos, size_t n, Consts k,
-                                                     const uint32_t *__restrict__ skey, const uint32_t *__restrict__ perm,
-                                                     const uint32_t *__restrict__ offset, const uint32_t *__restrict__ poff,
-                                                     float *__restrict__ X, float *__restrict__ Y, float *__restrict__ Z)
+template <int BITS>
+static cudaError_t scatter_dispatch(bool iota, bool last, const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout,
+                                    size_t n, int shift, const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st)
 {
-    size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
-    const uint32_t c = skey[s];
-    const size_t i = perm[s];
-    const uint32_t cz = c % k.cpd, cy = (c / k.cpd) % k.cpd, cx = c / (k.cpd * k.cpd);
-    // corner origins are float32 values; pos - origin is exact (Sterbenz), the power-of-two scale too
-    const float ox = (float)((double)cx * k.cell_w), oy = (float)((double)cy * k.cell_w), oz = (float)((double)cz * k.cell_w);
-    const float sc = (float)k.scale;
-    const uint32_t o0 = offset[c], o1 = offset[c + 1];
-    const uint32_t p = poff[c] + (uint32_t)(s - o0);
-    X[p] = (pos[3 * i + 0] - ox) * sc;
-    Y[p] = (pos[3 * i + 1] - oy) * sc;
-    Z[p] = (pos[3 * i + 2] - oz) * sc;
-    if (s + 1 == o1) {
-        const uint32_t pe = poff[c + 1];
-        for (uint32_t q = p + 1; q < pe; q++) { X[q] = kDummy; Y[q] = kDummy; Z[q] = kDummy; }
+    if (iota) return last ? scatter_launch<BITS, true, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st)
+                          : scatter_launch<BITS, true, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st);
+    return last ? scatter_launch<BITS, false, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st)
+                : scatter_launch<BITS, false, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st);
+}
+
+// One pass over n keys: digit histogram per tile (unless the caller already has it), its scan, the scatter.
+// `last` (particle sort only) fuses the gather of `g` into the scatter.
+static int radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift, int bits,
+                      bool iota, bool last, bool have_hist, const GatherArgs &g, uint32_t *hist, uint32_t *scan_tmp,
+                      cudaStream_t st, int *launches)
+{
+    const uint32_t nb = (uint32_t)((n + kSortTile - 1) / kSortTile);
+    const uint32_t bins = 1u << bits;
+    if (!have_hist) {
+        radix_hist_kernel<<<nb, kSortThreads, 0, st>>>(kin, n, shift, bins - 1u, hist, nb);
+        *launches += 1;
     }
+    exclusive_scan(hist, hist, (size_t)bins * nb, scan_tmp, OpId(), 0, nullptr, st, launches);
+    cudaError_t e;
+    switch (bits) {
+    case 8:  e = scatter_dispatch<8>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
+    case 9:  e = scatter_dispatch<9>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
+    case 10: e = scatter_dispatch<10>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
+    default: e = scatter_dispatch<11>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
+    }
+    NF_CUDA_OK(e);
+    *launches += 1;
+    return NF_OK;
 }
 
 // ---- S5: stencil source counts, work units, cost keys, exact interaction count -------------------------------
@@ -341,35 +513,37 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     int L = 0;
     p->have_bin_time = false;
     p->n_units = 0;
-    if (n == 0) { p->launches_bin = 0; p->perm = ws.valA; p->sorted_keys = ws.keyA; return NF_OK; }
+    if (n == 0) { p->launches_bin = 0; p->perm = ws.valA; return NF_OK; }
 
     NF_CUDA_OK(cudaEventRecord(p->ev[0], st));
     NF_CUDA_OK(cudaMemsetAsync(ws.count, 0, 4 * (size_t)(k.ncells + 1), st));
     NF_CUDA_OK(cudaMemsetAsync(ws.scalars, 0, 4 * 64, st));
     NF_CUDA_OK(cudaMemsetAsync(ws.interactions, 0, 8, st));
 
-    const unsigned nb256 = (unsigned)((n + 255) / 256);
-    cellid_kernel<<<nb256, 256, 0, st>>>(pos, n, k, ws.cid, ws.count, ws.scalars);  L++;
+    // stable sort by cell id: the first pass's digit histogram comes out of the cell-id kernel, the last pass writes
+    // perm and the padded SoA arrays (no sorted keys are stored)
+    int passes = 1, dbits = kSortMinBits;
+    sort_plan((unsigned long long)k.ncells, &passes, &dbits);
+    const uint32_t nbs = (uint32_t)((n + kSortTile - 1) / kSortTile);
+    cellid_kernel<<<nbs, kSortThreads, 0, st>>>(pos, n, k, ws.cid, ws.count, ws.scalars, (1u << dbits) - 1u, ws.radix_hist, nbs);  L++;
 
     // prefix sums: offset (exported), padded offsets, unit bases
     exclusive_scan(ws.count, ws.offset, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
     exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
 
-    // stable sort by cell id
-    int bits = 1;
-    while (bits < 32 && (1ull << bits) < (unsigned long long)k.ncells) bits++;
-    const int passes = (bits + 7) / 8;
+    GatherArgs g;
+    g.pos = pos; g.offset = ws.offset; g.poff = ws.poff; g.X = ws.x; g.Y = ws.y; g.Z = ws.z; g.k = k;
     const uint32_t *kin = ws.cid, *vin = nullptr;
     uint32_t *kbuf[2] = {ws.keyA, ws.keyB}, *vbuf[2] = {ws.valA, ws.valB};
     for (int ps = 0; ps < passes; ps++) {
-        radix_pass(kin, vin, kbuf[ps & 1], vbuf[ps & 1], n, 8 * ps, ps == 0, ws.radix_hist, ws.scan_tmp, st, &L);
+        const int rc = radix_pass(kin, vin, kbuf[ps & 1], vbuf[ps & 1], n, dbits * ps, dbits, ps == 0, ps == passes - 1, ps == 0, g,
+                                  ws.radix_hist, ws.scan_tmp, st, &L);
+        if (rc != NF_OK) return rc;
         kin = kbuf[ps & 1]; vin = vbuf[ps & 1];
     }
     p->sort_passes = passes;
-    p->sorted_keys = kin; p->perm = vin;
+    p->perm = vin;
     uint32_t *free_key = kbuf[passes & 1], *free_val = vbuf[passes & 1];   // the pair not holding the result
-
-    gather_kernel<<<nb256, 256, 0, st>>>(pos, n, k, p->sorted_keys, p->perm, ws.offset, ws.poff, ws.x, ws.y, ws.z);  L++;
 
     // stencil source counts + exact interaction count, units per column, units + heavy-first order: one
     // stable radix pass on the cost key (clz of the unit's interaction count, so heavier units come first
@@ -392,7 +566,9 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     const size_t nu = sc[2];
     p->n_units = (long long)nu;
     if (p->heavy_first && nu > 1) {
-        radix_pass(ukey, nullptr, free_key, free_val, nu, 0, true, ws.radix_hist, ws.scan_tmp, st, &L);
+        const int rc = radix_pass(ukey, nullptr, free_key, free_val, nu, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
+                                  ws.scan_tmp, st, &L);
+        if (rc != NF_OK) return rc;
         units_permute_kernel<<<(unsigned)((nu + 255) / 256), 256, 0, st>>>(ws.units, free_val, &ws.scalars[2], ws.units_sorted);  L++;
     } else if (nu > 0) {
         NF_CUDA_OK(cudaMemcpyAsync(ws.units_sorted, ws.units, sizeof(Unit) * nu, cudaMemcpyDeviceToDevice, st));

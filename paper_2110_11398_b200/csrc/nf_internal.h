@@ -38,10 +38,23 @@ constexpr unsigned kWaitSleepNs = NF_WAIT_SLEEP_NS;  // back-off of a waiting wa
 constexpr float kDummy       = 36028797018963968.0f;        // 2^55: pad-slot coordinate, contributes exactly 0
 
 // ---- radix sort shape ----------------------------------------------------------------------
-constexpr int kSortWarps   = 8;
+constexpr int kSortWarps   = 16;
 constexpr int kSortThreads = 32 * kSortWarps;
 constexpr int kSortItems   = 16;                          // keys per thread
-constexpr int kSortTile    = kSortThreads * kSortItems;   // 4096 keys per block
+constexpr int kSortTile    = kSortThreads * kSortItems;   // 8192 keys per block
+constexpr int kSortMinBits = 8, kSortMaxBits = 11;        // digit width of one pass
+
+// LSD passes and digit width for keys below `nkeys` (cell ids: nkeys = cpd^3): as few passes as 11-bit digits allow,
+// the bits spread evenly over them (18 bits: 2 x 9; 21: 2 x 11; 24: 3 x 8)
+inline void sort_plan(unsigned long long nkeys, int *passes, int *digit_bits)
+{
+    int bits = 1;
+    while (bits < 32 && (1ull << bits) < nkeys) bits++;
+    const int np = (bits + kSortMaxBits - 1) / kSortMaxBits;
+    int b = (bits + np - 1) / np;
+    if (b < kSortMinBits) b = kSortMinBits;
+    *passes = np; *digit_bits = b;
+}
 
 struct Unit {            // one work unit: a window of <= kChunk consecutive cell-sorted sinks of one z-column
     uint32_t s0;         // first sorted slot (index into perm)
@@ -53,7 +66,7 @@ struct Unit {            // one work unit: a window of <= kChunk consecutive cel
 
 struct Workspace {       // carved out of one arena; all 256-byte aligned
     uint32_t *cid, *keyA, *keyB, *valA, *valB;   // [n]
-    uint32_t *radix_hist;                         // [256 * sort_blocks]
+    uint32_t *radix_hist;                         // [bins * sort_blocks], digit-major
     uint32_t *count, *offset, *poff, *ubase;      // [C], [C+1], [C+1], [cpd^2+1] (unit base per column)
     uint32_t *src;                                // [C] particles in the stencil of each cell
     uint32_t *scan_tmp;                           // block sums
@@ -97,7 +110,7 @@ struct nf_plan {
     long long n;  bool binned;
     long long n_units;
     int sort_passes;
-    const uint32_t *perm, *sorted_keys;
+    const uint32_t *perm;
     // host-buffer path
     float *pos_stage; float *acc_stage; size_t stage_cap;   // device staging for *_host calls
     // options

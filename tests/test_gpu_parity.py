@@ -250,6 +250,39 @@ def test_layout_is_lossless():
     assert np.all(lay["x"].cpu().numpy()[~real] == 2.0 ** 55)
 
 
+@pytest.mark.parametrize("cpd,n", [(9, 40_000), (16, 100_001), (26, 8192), (63, 300_000), (90, 250_000), (125, 400_000),
+                                   (203, 300_000), (255, 16_385)])
+def test_binning_digit_widths(oracle_mod, cpd, n):
+    """The sort takes 1-3 passes of 8-11 bit digits depending on cpd^3 (10 bits x 1 ... 8 bits x 3): binning arrays
+    bit-exact against the oracle and the padded SoA layout lossless, on uniform positions with a block of
+    particles in one cell (ties over many tiles) and ragged last tiles."""
+    import paper_2110_11398_b200 as nf
+    rng = np.random.default_rng(cpd * 1000 + 7)
+    pos = rng.random((n, 3), dtype=np.float32)
+    pos[n // 3: n // 3 + n // 5] = np.float32(0.5) + rng.random((n // 5, 3), dtype=np.float32) * np.float32(0.2 / cpd)
+    pos = pos[rng.permutation(n)]
+    ref = oracle_mod.bin_particles(pos, cpd, 1.0)
+    with nf.Plan(cpd, 1.0, 1e-4, 2) as p:
+        p.bin(torch.from_numpy(pos).cuda())
+        b = {k: u32(v) for k, v in p.binning().items()}
+        lay = p.layout()
+        lay = {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in lay.items()}
+    assert_binning_equal(b, ref)
+    poff = lay["poff"].view(np.uint32).astype(np.int64)
+    cnt = ref["count"].astype(np.int64)
+    assert np.array_equal(np.diff(poff), (cnt + 3) // 4 * 4)
+    cid_sorted = np.repeat(np.arange(cpd ** 3), cnt)
+    slot = np.repeat(poff[:-1], cnt) + (np.arange(n) - np.repeat(ref["offset"][:-1].astype(np.int64), cnt))
+    p64 = pos.astype(np.float64)[ref["perm"]]
+    for d, (name, cidx) in enumerate(zip("xyz", [cid_sorted // cpd ** 2, (cid_sorted // cpd) % cpd, cid_sorted % cpd])):
+        corner = (cidx.astype(np.float64) * (1.0 / cpd)).astype(np.float32).astype(np.float64)
+        rec = lay[name].astype(np.float64)[slot] / lay["scale"] + corner
+        assert np.array_equal(rec, p64[:, d]), name
+        real = np.zeros(poff[-1], bool)
+        real[slot] = True
+        assert np.all(lay[name][:poff[-1]][~real] == 2.0 ** 55), name
+
+
 def test_rebin_workspace_stream(oracle_mod):
     """nf_bin may be called repeatedly with new n; caller-lent workspace; non-default stream."""
     import paper_2110_11398_b200 as nf

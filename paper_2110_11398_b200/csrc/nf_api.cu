@@ -37,7 +37,7 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     const size_t nonempty = N < C ? N : C;
     const size_t pmax = N + 3 * nonempty + 8;
     const size_t ncol = (size_t)cpd * cpd;
-    const size_t umax = (N < ncol ? N : ncol) + N / kChunk + 2;    // every column ends with one ragged window
+    const size_t umax = (N < ncol ? N : ncol) + N / 32 + 2;    // every column ends with one ragged window; windows >= 32 sinks
     const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
     int sort_passes = 1, sort_bits = kSortMinBits;
     sort_plan((unsigned long long)C, &sort_passes, &sort_bits);
@@ -200,7 +200,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     memset(p, 0, sizeof(*p));
     Consts &k = p->k;
     k.cpd = cpd; k.R = R; k.ncells = (uint32_t)cpd * cpd * cpd;
-    k.slab0 = 0; k.nslab = cpd;
+    k.slab0 = 0; k.nslab = cpd; k.chunk = kChunk;
     k.L = L; k.cell_w = L / cpd; k.inv_cell_w = (double)cpd / L;
     int e2 = 0;
     (void)std::frexp(k.cell_w, &e2);              // cell_w = m 2^e2, m in [0.5, 1)
@@ -211,7 +211,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     p->device = -1;
     p->stream = 0;
     p->ws_n = -1;
-    p->variant = 0; p->fastpath = 1; p->heavy_first = 1; p->ctas_per_sm = 0;
+    p->variant = 0; p->fastpath = 1; p->heavy_first = 1; p->ctas_per_sm = 0; p->window = 0;
     g_err[0] = 0;
     return p;
 }
@@ -413,6 +413,9 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
         return set_softening(p, (int)v);
     }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
+    if (!strcmp(key, "window") && (v == 0 || v == 32 || v == 64 || v == 128 || v == 256) && v <= kChunk) {
+        p->window = (int)v; p->binned = false; return NF_OK;
+    }
     set_error("unknown option or bad value: %s = %lld", key, v);
     return NF_ERR_ARG;
 }

@@ -459,7 +459,7 @@ __global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t 
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
     const uint32_t ncol = offset[(size_t)(col + 1) * k.cpd] - offset[(size_t)col * k.cpd];
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
-    nunits[col] = rel < k.nslab ? (ncol + kChunk - 1) / kChunk : 0u;            // columns outside the sink slabs: sources only
+    nunits[col] = rel < k.nslab ? (ncol + k.chunk - 1) / k.chunk : 0u;            // columns outside the sink slabs: sources only
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
@@ -476,8 +476,8 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
     const uint32_t c_begin = off[0], c_end = off[k.cpd];
     uint32_t u = ubase[col];
     int z = 0;
-    for (uint32_t s0 = c_begin; s0 < c_end; s0 += kChunk, u++) {
-        const uint32_t s1 = min(s0 + (uint32_t)kChunk, c_end);
+    for (uint32_t s0 = c_begin; s0 < c_end; s0 += k.chunk, u++) {
+        const uint32_t s1 = min(s0 + (uint32_t)k.chunk, c_end);
         while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
         Unit un;
         un.s0 = s0; un.col = col; un.ns = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
@@ -507,6 +507,7 @@ __global__ void __launch_bounds__(256) units_permute_kernel(const Unit *__restri
 int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 {
     const size_t n = (size_t)n_ll;
+    p->k.chunk = p->window > 0 ? p->window : kChunk;      // sinks per work unit
     const Consts &k = p->k;
     Workspace &ws = p->ws;
     cudaStream_t st = p->stream;

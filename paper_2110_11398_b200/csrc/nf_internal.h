@@ -80,6 +80,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
 
 struct Consts {          // everything the kernels need about the problem, by value
     int cpd, R;
+    int chunk;                      // sinks per work unit (window of one z-column), 32..kChunk
     int slab0, nslab;               // sink slabs: cells with x index in {slab0, ..., slab0 + nslab - 1} mod cpd (default: all)
     uint32_t ncells;
     double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L
@@ -114,7 +115,7 @@ struct nf_plan {
     // host-buffer path
     float *pos_stage; float *acc_stage; size_t stage_cap;   // device staging for *_host calls
     // options
-    int variant, fastpath, heavy_first, ctas_per_sm;
+    int variant, fastpath, heavy_first, ctas_per_sm, window;
     // stats
     cudaEvent_t ev[4];
     bool have_bin_time, have_accel_time;

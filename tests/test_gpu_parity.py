@@ -513,6 +513,7 @@ def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, worl
     cfg = nf_inputs.scaled(idx, n_side, cpd)
     pos = nf_inputs.generate(cfg)
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.set_option("window", 64)       # any window: equal on every plan
         plan.bin(pos.cuda())
         whole = plan.accel().cpu()
         total = plan.stats()["interactions"]
@@ -528,6 +529,7 @@ def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, worl
         local = torch.cat([owned[r]] + halos).contiguous()
         with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
             plan.set_sink_slabs(f, c)
+            plan.set_option("window", 64)
             plan.bin(local.cuda())
             acc = torch.full((local.shape[0], 3), 7.0, device="cuda")
             plan.accel(acc)
@@ -600,6 +602,31 @@ def test_bitwise_determinism():
             outs.append((a1, a2.clone(), rho.clone()))
     for o in outs[1:]:
         assert all(torch.equal(x, y) for x, y in zip(o, outs[0]))
+
+
+@pytest.mark.parametrize("idx,n_side,cpd", [(1, 32, 9), (4, 40, 10)])
+def test_window_sizes(oracle_mod, idx, n_side, cpd):
+    """Sinks per work unit ("window": 32..256, 0 = the default 256): every choice within tolerance of the
+    oracle, same interaction count, bit-identical for equal windows; bad values are rejected."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
+    counts, units = set(), {}
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
+        for w in (0, 32, 64, 128, 256, 64):
+            p.set_option("window", w)
+            p.bin(pos.cuda())
+            a = p.accel().cpu()
+            st = p.stats()
+            counts.add(st["interactions"])
+            assert_parity(a.numpy().astype(np.float64), ref, f"{cfg.name} window {w}")
+            if w in units:
+                assert torch.equal(units[w], a)
+            units[w] = a
+        with pytest.raises(nf.NFError):
+            p.set_option("window", 48)
+    assert len(counts) == 1
 
 
 def test_config4_full_size_density_and_kick_sampled(oracle_mod):

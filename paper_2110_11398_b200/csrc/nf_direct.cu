@@ -105,6 +105,19 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 // ---- pair bodies -------------------------------------------------------------------------------
 struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin)
 
+// a += k d for two packed interactions.  A packed FFMA2 with three distinct register-pair operands holds the
+// register-file read ports 3 cycles for 2 cycles of pipe; NF_SCALAR_ACC of the three components (x, y, z order)
+// are issued as two scalar FFMA instead (2 cycles, one more issue slot each).
+#ifndef NF_SCALAR_ACC
+#define NF_SCALAR_ACC 0
+#endif
+template <int COMP>
+__device__ __forceinline__ void accum2(const float2 k, const float2 d, float2 &a)
+{
+    if (COMP < NF_SCALAR_ACC) { a.x = fmaf(k.x, d.x, a.x); a.y = fmaf(k.y, d.y, a.y); }
+    else a = __ffma2_rn(k, d, a);
+}
+
 // two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
 // (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ
 __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
@@ -119,9 +132,9 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
     ri.y = rsqrt_approx(r2.y);
     const float2 ri2 = __fmul2_rn(ri, ri);
     const float2 k = __fmul2_rn(ri2, ri);
-    ax = __ffma2_rn(k, dx, ax);
-    ay = __ffma2_rn(k, dy, ay);
-    az = __ffma2_rn(k, dz, az);
+    accum2<0>(k, dx, ax);
+    accum2<1>(k, dy, ay);
+    accum2<2>(k, dz, az);
 }
 
 // scalar body (variant 1): 14 / 11 FP32-pipe instructions per interaction (+ 3 with the density estimate).
@@ -225,8 +238,8 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
             pair_density(r2a, c, f.rho);
             pair_density(r2b, c, f.rho);
         }
-        f.x = __ffma2_rn(ka, dxa, f.x); f.y = __ffma2_rn(ka, dya, f.y); f.z = __ffma2_rn(ka, dza, f.z);
-        f.x = __ffma2_rn(kb, dxb, f.x); f.y = __ffma2_rn(kb, dyb, f.y); f.z = __ffma2_rn(kb, dzb, f.z);
+        accum2<0>(ka, dxa, f.x); accum2<1>(ka, dya, f.y); accum2<2>(ka, dza, f.z);
+        accum2<0>(kb, dxb, f.x); accum2<1>(kb, dyb, f.y); accum2<2>(kb, dzb, f.z);
     } else {
         interact1<MODE>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
         interact1<MODE>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);

@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--fastpath", type=int, default=None)
     ap.add_argument("--heavy-first", type=int, default=None)
     ap.add_argument("--ctas-per-sm", type=int, default=None)
+    ap.add_argument("--window", type=int, default=None, help="sinks per work unit (nf_set_option window)")
     return ap.parse_args()
 
 
@@ -156,7 +157,7 @@ def fp32_peak_tflops(stats):
 
 def apply_options(plan, args):
     for key, val in (("variant", args.variant), ("fastpath", args.fastpath), ("heavy_first", args.heavy_first),
-                     ("ctas_per_sm", args.ctas_per_sm)):
+                     ("ctas_per_sm", args.ctas_per_sm), ("window", args.window)):
         if val is not None:
             plan.set_option(key, val)
 

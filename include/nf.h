@@ -192,7 +192,7 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
- *   "window"       sinks per work unit: 0 = 256 (default), or 32 / 64 / 128 / 256.  Shorter windows give a small
+ *   "window"       sinks per work unit: 0 = 256 (default), or a multiple of 32 up to 256.  Shorter windows give a small
  *                  problem more work units but every unit streams its whole stencil again (measured slower on
  *                  config 1).  Accelerations are bit-identical between plans only for equal
  *                  windows.  Takes effect at the next nf_bin.

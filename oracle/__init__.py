@@ -10,6 +10,7 @@ from .nf_oracle import (  # noqa: F401
     kernel,
     bin_particles,
     accel,
+    accel_mass,
     density,
     kick,
     cell_max_accel,

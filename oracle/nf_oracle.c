@@ -201,6 +201,57 @@ int nfo_accel(const float *pos, int64_t n, int cpd, double L, double eps, int R,
 }
 
 /*
+ * Variant with per-particle masses (the paper's particles all have one mass, PAPER.md:27,117,
+ * so this is the same direct sum of PAPER.md:349 with the source mass written out instead of set to 1, reading C4):
+ *   a_i = sum_j m_j d_ij K(|d_ij|),  G = 1, the sink's own mass does not enter.
+ * Written out on its own (not by calling nfo_one_sink) so that the unit-mass oracle stays as it was pinned;
+ * mass [n] float32 in input order, converted to float64 like the positions.
+ */
+int nfo_accel_mass(const float *pos, const float *mass, int64_t n, int cpd, double L, double eps, int R, int kind,
+                   const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
+                   const int64_t *sinks, int64_t m, double *acc)
+{
+    if (kind != 0 && kind != 1) return NFO_ERR_ARG;
+    if (nfo_check_args(cpd, L, eps, R) != NFO_OK || n < 0 || m < 0 || !mass) return NFO_ERR_ARG;
+    if (!sinks && m != n) return NFO_ERR_ARG;
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(|:bad)
+    for (int64_t k = 0; k < m; k++) {
+        int64_t i = sinks ? sinks[k] : k;
+        if (i < 0 || i >= n) { bad |= 1; continue; }
+        uint32_t id = cid[i];
+        int cz = (int)(id % (uint32_t)cpd);
+        int cy = (int)((id / (uint32_t)cpd) % (uint32_t)cpd);
+        int cx = (int)(id / ((uint32_t)cpd * (uint32_t)cpd));
+        double xi = (double)pos[3 * i + 0], yi = (double)pos[3 * i + 1], zi = (double)pos[3 * i + 2];
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        for (int ox = -R; ox <= R; ox++)
+        for (int oy = -R; oy <= R; oy++)
+        for (int oz = -R; oz <= R; oz++) {
+            int sx = cx + ox, sy = cy + oy, sz = cz + oz;
+            double wx = 0.0, wy = 0.0, wz = 0.0;
+            if (sx < 0) { sx += cpd; wx = -1.0; } else if (sx >= cpd) { sx -= cpd; wx = 1.0; }
+            if (sy < 0) { sy += cpd; wy = -1.0; } else if (sy >= cpd) { sy -= cpd; wy = 1.0; }
+            if (sz < 0) { sz += cpd; wz = -1.0; } else if (sz >= cpd) { sz -= cpd; wz = 1.0; }
+            int64_t c2 = ((int64_t)sx * cpd + sy) * cpd + sz;
+            for (uint32_t t = offset[c2]; t < offset[c2 + 1]; t++) {
+                int64_t j = perm[t];
+                double dx = (double)pos[3 * j + 0] - xi + wx * L;
+                double dy = (double)pos[3 * j + 1] - yi + wy * L;
+                double dz = (double)pos[3 * j + 2] - zi + wz * L;
+                double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 == 0.0) continue;
+                double K = kind == 1 ? nfo_kernel_plummer(sqrt(r2), eps) : nfo_kernel(sqrt(r2), eps);
+                double mK = (double)mass[j] * K;
+                ax += dx * mK; ay += dy * mK; az += dz * mK;
+            }
+        }
+        acc[3 * k + 0] = ax; acc[3 * k + 1] = ay; acc[3 * k + 2] = az;
+    }
+    return bad ? NFO_ERR_ARG : NFO_OK;
+}
+
+/*
  * Kernel density estimate, computed by the paper "as part of the near-field force computation":
  * "a kernel density estimate around all particles, using a weighting of 1 - r^2/b^2, where b is chosen
  * to be 40% of the interparticle spacing" (sec. 3.3).

@@ -46,6 +46,8 @@ def _load():
         lib.nfo_kernel_plummer.argtypes = [f64, f64]
         lib.nfo_accel_kind.restype = i32
         lib.nfo_accel_kind.argtypes = [vp, i64, i32, f64, f64, i32, i32, vp, vp, vp, vp, i64, vp]
+        lib.nfo_accel_mass.restype = i32
+        lib.nfo_accel_mass.argtypes = [vp, vp, i64, i32, f64, f64, i32, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_accel.restype = i32
         lib.nfo_accel.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_density.restype = i32
@@ -113,6 +115,31 @@ def accel(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=N
                            binning["cid"].ctypes.data, binning["offset"].ctypes.data,
                            binning["perm"].ctypes.data, sp, m, acc.ctypes.data)
     _check(rc, "nfo_accel")
+    return acc
+
+
+def accel_mass(pos, mass, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=None,
+               softening: str = "spline") -> np.ndarray:
+    """float64 accelerations [m][3] with per-particle source masses: a_i = sum_j m_j d_ij K(r_ij)
+    (the direct sum of PAPER.md:349 with the mass written out; ``mass`` float32 [n], input order)."""
+    kind = {"spline": 0, "plummer": 1}[softening]
+    pos = _pos32(pos)
+    n = pos.shape[0]
+    mass = np.ascontiguousarray(mass, dtype=np.float32)
+    if mass.shape != (n,):
+        raise ValueError("mass must have shape (n,)")
+    if binning is None:
+        binning = bin_particles(pos, cpd, L)
+    if sinks is None:
+        sp, m = None, n
+    else:
+        sinks = np.ascontiguousarray(sinks, dtype=np.int64)
+        sp, m = sinks.ctypes.data, sinks.shape[0]
+    acc = np.zeros((m, 3), np.float64)
+    rc = _load().nfo_accel_mass(pos.ctypes.data, mass.ctypes.data, n, cpd, float(L), float(eps), int(R), kind,
+                                binning["cid"].ctypes.data, binning["offset"].ctypes.data,
+                                binning["perm"].ctypes.data, sp, m, acc.ctypes.data)
+    _check(rc, "nfo_accel_mass")
     return acc
 
 

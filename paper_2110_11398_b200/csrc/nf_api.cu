@@ -413,7 +413,7 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
         return set_softening(p, (int)v);
     }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
-    if (!strcmp(key, "window") && (v == 0 || v == 32 || v == 64 || v == 128 || v == 256) && v <= kChunk) {
+    if (!strcmp(key, "window") && v >= 0 && v % 32 == 0 && v <= kChunk) {
         p->window = (int)v; p->binned = false; return NF_OK;
     }
     set_error("unknown option or bad value: %s = %lld", key, v);

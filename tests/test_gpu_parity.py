@@ -606,7 +606,7 @@ def test_bitwise_determinism():
 
 @pytest.mark.parametrize("idx,n_side,cpd", [(1, 32, 9), (4, 40, 10)])
 def test_window_sizes(oracle_mod, idx, n_side, cpd):
-    """Sinks per work unit ("window": 32..256, 0 = the default 256): every choice within tolerance of the
+    """Sinks per work unit ("window": multiples of 32 up to 256, 0 = the default 256): every choice within tolerance of the
     oracle, same interaction count, bit-identical for equal windows; bad values are rejected."""
     import paper_2110_11398_b200 as nf
     cfg = nf_inputs.scaled(idx, n_side, cpd)
@@ -614,7 +614,7 @@ def test_window_sizes(oracle_mod, idx, n_side, cpd):
     ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
     counts, units = set(), {}
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
-        for w in (0, 32, 64, 128, 256, 64):
+        for w in (0, 32, 64, 96, 128, 224, 256, 64):
             p.set_option("window", w)
             p.bin(pos.cuda())
             a = p.accel().cpu()

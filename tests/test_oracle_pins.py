@@ -500,3 +500,93 @@ def test_plummer_brute_force(oracle_mod, cpd, R, n, eps):
     ref = (d * k[..., None]).sum(1)
     np.testing.assert_allclose(a, ref, rtol=1e-9, atol=1e-9 * np.abs(ref).max())
     assert np.abs(a.sum(0)).max() <= 1e-10 * np.abs(a).sum()
+
+
+# ------------------------------------------------------------------ per-particle masses
+def test_mass_two_body_closed_form(oracle_mod):
+    """Dyadic two-body case outside the spline radius: |a_1| = m_2 / d^2 towards 2, |a_2| = m_1 / d^2 towards 1
+    (Newton, G = 1); the sink's own mass does not enter.  d = 1/4, m = (3, 1/2): a_1 = +8, a_2 = -48 exactly."""
+    pos = np.array([[0.25, 0.5, 0.5], [0.5, 0.5, 0.5]], np.float32)
+    mass = np.array([3.0, 0.5], np.float32)
+    a = oracle_mod.accel_mass(pos, mass, 8, 1.0, 1.0 / 256, 2)
+    assert a[0].tolist() == [8.0, 0.0, 0.0] and a[1].tolist() == [-48.0, 0.0, 0.0]
+    # inside the spline the same factor multiplies the unit-mass closed form d (10 - 15u + 6u^2) / eps_s^3
+    eps = 0.125 / 2.16 * 2.0                           # eps_s = 0.25: d = 1/8 is u = 1/2
+    pos = np.array([[0.5, 0.5, 0.5], [0.625, 0.5, 0.5]], np.float32)
+    a = oracle_mod.accel_mass(pos, mass, 8, 1.0, eps, 2)
+    f = 0.125 * (10 - 7.5 + 1.5) / (2.16 * eps) ** 3
+    assert a[0, 0] == pytest.approx(0.5 * f, rel=1e-14) and a[1, 0] == pytest.approx(-3.0 * f, rel=1e-14)
+
+
+@pytest.mark.parametrize("softening", ["spline", "plummer"])
+def test_mass_reduces_to_unit_and_is_linear(oracle_mod, softening):
+    rng = np.random.default_rng(5)
+    n, cpd, eps = 600, 6, 0.02
+    pos = rng.random((n, 3), dtype=np.float32)
+    unit = oracle_mod.accel(pos, cpd, 1.0, eps, 2, softening=softening)
+    ones = oracle_mod.accel_mass(pos, np.ones(n, np.float32), cpd, 1.0, eps, 2, softening=softening)
+    assert np.array_equal(unit, ones)                                    # m = 1: the pinned oracle, bit for bit
+    m1 = rng.random(n, dtype=np.float32) + 0.5
+    m2 = rng.random(n, dtype=np.float32)
+    a1 = oracle_mod.accel_mass(pos, m1, cpd, 1.0, eps, 2, softening=softening)
+    a2 = oracle_mod.accel_mass(pos, m2, cpd, 1.0, eps, 2, softening=softening)
+    assert np.array_equal(oracle_mod.accel_mass(pos, 4 * m1, cpd, 1.0, eps, 2, softening=softening), 4 * a1)   # power of two: exact
+    m12 = (m1.astype(np.float64) + m2).astype(np.float32)
+    keep = m12.astype(np.float64) == m1.astype(np.float64) + m2            # sums exact in float32
+    both = oracle_mod.accel_mass(pos, np.where(keep, m12, 0).astype(np.float32), cpd, 1.0, eps, 2, softening=softening)
+    sep = oracle_mod.accel_mass(pos, np.where(keep, m1, 0).astype(np.float32), cpd, 1.0, eps, 2, softening=softening) + \
+          oracle_mod.accel_mass(pos, np.where(keep, m2, 0).astype(np.float32), cpd, 1.0, eps, 2, softening=softening)
+    np.testing.assert_allclose(both, sep, rtol=1e-11, atol=1e-11 * np.abs(both).max())   # superposition
+    assert keep.sum() > n // 4
+
+
+def test_mass_momentum_conservation_and_test_particles(oracle_mod):
+    """sum_i m_i a_i = 0 (pair antisymmetry with the symmetric stencil); a massless particle feels the others but
+    changes nothing for them: dropping it from the input leaves every other acceleration as it was."""
+    rng = np.random.default_rng(6)
+    n, cpd, eps = 500, 7, 0.03
+    pos = rng.random((n, 3), dtype=np.float32)
+    mass = rng.lognormal(0.0, 1.0, n).astype(np.float32)
+    a = oracle_mod.accel_mass(pos, mass, cpd, 1.0, eps, 2)
+    mom = (mass.astype(np.float64)[:, None] * a).sum(0)
+    assert np.abs(mom).max() <= 1e-12 * np.abs(mass[:, None] * a).sum()
+    ghost = rng.random(n) < 0.2
+    m0 = np.where(ghost, 0, mass).astype(np.float32)
+    full = oracle_mod.accel_mass(pos, m0, cpd, 1.0, eps, 2)
+    sub = oracle_mod.accel_mass(pos[~ghost], m0[~ghost], cpd, 1.0, eps, 2)
+    np.testing.assert_allclose(full[~ghost], sub, rtol=1e-12, atol=1e-12 * np.abs(sub).max())
+    assert np.linalg.norm(full[ghost], axis=1).min() > 0
+
+
+def test_mass_equals_coincident_unit_particles(oracle_mod):
+    """Independent route through the UNIT-mass oracle: a particle of integer mass k acts on all others like k unit
+    particles at the same point (which exert nothing on each other: r = 0 contributes 0, reading C5)."""
+    rng = np.random.default_rng(7)
+    n, cpd, eps = 300, 6, 0.02
+    pos = rng.random((n, 3), dtype=np.float32)
+    k = rng.integers(1, 5, n)
+    a = oracle_mod.accel_mass(pos, k.astype(np.float32), cpd, 1.0, eps, 2)
+    rep = np.repeat(np.arange(n), k)
+    unit = oracle_mod.accel(pos[rep], cpd, 1.0, eps, 2)
+    first = np.concatenate([[0], np.cumsum(k)[:-1]])
+    np.testing.assert_allclose(a, unit[first], rtol=1e-12, atol=1e-12 * np.abs(a).max())
+
+
+@pytest.mark.parametrize("cpd,R,n,eps", [(6, 2, 350, 0.02), (5, 2, 250, 0.05), (4, 1, 200, 0.0)])
+def test_mass_brute_force(oracle_mod, cpd, R, n, eps):
+    """All pairs in numpy with the kernel built from its defining property (taylor_kernel), explicit cell-offset mask;
+    cpd = 2R+1 included (image by cell offset, every cell seen once)."""
+    rng = np.random.default_rng(n + 1)
+    pos = rng.random((n, 3), dtype=np.float32)
+    mass = (rng.random(n) * 3 + 0.1).astype(np.float32)
+    a = oracle_mod.accel_mass(pos, mass, cpd, 1.0, eps, R)
+    p = pos.astype(np.float64)
+    c = cells_of(pos, cpd, 1.0)
+    off = (c[None] - c[:, None] + R) % cpd - R               # source cell - sink cell, wrapped into [-R, cpd-1-R]
+    near = (np.abs(off) <= R).all(-1)
+    w = (c[:, None] + off - c[None]) // cpd                  # box wrap implied by the cell offset (C7)
+    d = p[None] - p[:, None] + w
+    r = np.sqrt((d ** 2).sum(-1))
+    kk = np.where(near, taylor_kernel(r, 2.16 * eps), 0.0) * mass.astype(np.float64)[None]
+    ref = (d * kk[..., None]).sum(1)
+    np.testing.assert_allclose(a, ref, rtol=1e-9, atol=1e-9 * np.abs(ref).max())

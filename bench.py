@@ -25,8 +25,8 @@ METRIC = "near_field_pair_interactions_per_s"
 UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
 FLOPS_EXECUTED_MIN = 19         # the Newtonian body (3 add + 6 fma + 2 mul + rsqrt) the kernel runs where no pair is inside eps_s
-# DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v5_direct_kernel.md)
-NCU_TRAFFIC_BYTES = {"config3_uniform_256": 961545472 + 659134976, "config4_halos_512": 18111688000 + 5377143000}
+# DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v7_final.md)
+NCU_TRAFFIC_BYTES = {"config3_uniform_256": 959502336 + 656173312, "config4_halos_512": 18112927000 + 5452417000}
 L2_BYTES = 126 * 1024 * 1024
 
 
@@ -298,6 +298,23 @@ def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, wa
             out["kick_ms_accel"] = evd[0].elapsed_time(evd[1]) / steps
             out["amax_global"] = float(amax.max().item())
             del vel, amax
+            # per-particle source masses (nf_set_masses; fourth staged array, one FMUL2 per pair)
+            mass = nf_inputs.masses(cfg, device="cuda")
+            evm = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            plan.set_masses(mass)
+            plan.accel(acc)
+            torch.cuda.synchronize()
+            evm[0].record()
+            plan.set_masses(mass)
+            evm[1].record()
+            for _ in range(steps):
+                plan.accel(acc)
+            evm[2].record()
+            torch.cuda.synchronize()
+            out["mass_ms_set"] = evm[0].elapsed_time(evm[1])
+            out["mass_ms_accel"] = evm[1].elapsed_time(evm[2]) / steps
+            plan.set_masses(None)
+            del mass
         if with_e2e:
             pos_h = torch.empty(pos.shape, dtype=pos.dtype, pin_memory=True)
             pos_h.copy_(pos)
@@ -393,6 +410,11 @@ def main_b200(args):
         line["fused_kick"] = {"call": "nf_accel_kick: v += a dt and per-cell max |a| in the epilogue (PAPER.md:353, 212)",
                               "ms_accel": r["kick_ms_accel"], "overhead_frac": r["kick_ms_accel"] / (ta * 1e3) - 1.0,
                               "max_accel": r["amax_global"]}
+    if "mass_ms_accel" in r:
+        line["masses"] = {"call": "nf_set_masses (log-normal masses, sigma_ln 1) + nf_accel",
+                          "ms_set_masses": r["mass_ms_set"], "ms_accel": r["mass_ms_accel"],
+                          "overhead_frac": r["mass_ms_accel"] / (ta * 1e3) - 1.0,
+                          "interactions_per_s": I / (r["mass_ms_accel"] / 1e3)}
     if r["clocks"].get("sm_mhz"):
         line["roofline"]["frac_at_sampled_clock"] = achieved / (peak * r["clocks"]["sm_mhz"] * 1e3 / st["clock_khz"])
     if not args.no_cpu_baseline and world == 1:

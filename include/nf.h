@@ -127,6 +127,21 @@ int nf_accel_density(nf_plan *plan, float *acc_dev, float *rho_dev, double b);
  */
 int nf_accel_kick(nf_plan *plan, float *acc_dev, float *vel_dev, double dt, float *amax_cell_dev);
 
+/*
+ * nf_set_masses -- per-particle SOURCE masses for the particles last binned (variant of SURVEY.md 8(f) NEXT 4;
+ * the paper's particles all carry one mass, which is the default m = 1):
+ *   a_i = sum_j m_j d_ij K(|d_ij|),  G = 1; the sink's own mass does not enter.
+ * Every later nf_accel / nf_accel_density / nf_accel_kick on this binning uses them (the density estimate of
+ * nf_accel_density stays the unweighted count-based sum of PAPER.md:387).
+ *   mass_dev  DEVICE pointer, [n] float32 in input order (finite), read during the call's kernel, not retained;
+ *             NULL = back to unit masses.
+ * The masses are gathered into a plan-owned device array in the internal source layout (4 bytes per padded slot,
+ * allocated at the first call, outside any lent workspace).  nf_bin resets the plan to unit masses: call
+ * nf_set_masses after every nf_bin.  Asynchronous on the plan's stream.
+ * Errors: NF_ERR_STATE (no binning), NF_ERR_NOMEM, NF_ERR_CUDA.
+ */
+int nf_set_masses(nf_plan *plan, const float *mass_dev);
+
 /* nf_destroy -- frees everything the plan allocated (never a caller workspace).  NULL-safe. */
 void nf_destroy(nf_plan *plan);
 
@@ -192,7 +207,8 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
- *   "window"       sinks per work unit: 0 = 256 (default), or a multiple of 32 up to 256.  Shorter windows give a small
+ *   "window"       sinks per work unit: a multiple of 32 up to 256, or 0 (default) = 256, except for problems whose
+ *                  units would not fill the grid once, which get the shortest window >= 96 that still runs in one wave.  Shorter windows give a small
  *                  problem more work units but every unit streams its whole stencil again (measured slower on
  *                  config 1).  Accelerations are bit-identical between plans only for equal
  *                  windows.  Takes effect at the next nf_bin.

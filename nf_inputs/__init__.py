@@ -193,3 +193,11 @@ def generate(cfg: NFConfig, device="cpu") -> torch.Tensor:
         pos = pos * cfg.L
         pos[pos >= cfg.L] = 0.0
     return pos.contiguous()
+
+
+def masses(cfg: NFConfig, device="cpu", sigma_ln: float = 1.0) -> torch.Tensor:
+    """float32 masses [N] for the per-particle-mass variant (nf_set_masses): log-normal with median 1 (two decades of
+    spread at sigma_ln = 1), seeded from the config; no arithmetic of the method in here."""
+    device = torch.device(device)
+    g = _gen(cfg.seed + 7919, device)
+    return torch.exp(sigma_ln * torch.randn(cfg.n, generator=g, device=device, dtype=torch.float32)).contiguous()

@@ -21,7 +21,7 @@ NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -
 _ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
 
 EXPORTS = [
-    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_masses", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
 ]
@@ -66,6 +66,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_accel_density.argtypes = [vp, vp, vp, dbl]
     lib.nf_accel_kick.restype = i32
     lib.nf_accel_kick.argtypes = [vp, vp, vp, dbl, vp]
+    lib.nf_set_masses.restype = i32
+    lib.nf_set_masses.argtypes = [vp, vp]
     lib.nf_set_sink_slabs.restype = i32
     lib.nf_set_sink_slabs.argtypes = [vp, i32, i32]
     lib.nf_destroy.restype = None
@@ -164,6 +166,15 @@ def nf_accel_kick(plan: int, acc: torch.Tensor | None, vel: torch.Tensor | None,
             raise TypeError("amax_cell must be a contiguous CUDA float32 tensor of shape [cpd^3]")
         pm = ctypes.c_void_p(amax_cell.data_ptr())
     _check(_lib.nf_accel_kick(plan, pa, pv, float(dt), pm))
+
+
+def nf_set_masses(plan: int, mass: torch.Tensor | None, n: int) -> None:
+    if mass is None:
+        _check(_lib.nf_set_masses(plan, None))
+        return
+    if not (mass.is_cuda and mass.dtype == torch.float32 and mass.is_contiguous() and mass.shape == (n,)):
+        raise TypeError("mass must be a contiguous CUDA float32 tensor of shape [n]")
+    _check(_lib.nf_set_masses(plan, ctypes.c_void_p(mass.data_ptr())))
 
 
 def nf_set_sink_slabs(plan: int, x_first: int, n_slabs: int) -> None:
@@ -273,6 +284,11 @@ class Plan:
         self._use_current_stream()
         nf_bin(self._h, pos)
         self.n = pos.shape[0]
+
+    def set_masses(self, mass: torch.Tensor | None):
+        """Source masses [n] (input order) of the particles last binned; None = unit masses.  nf_bin resets them."""
+        self._use_current_stream()
+        nf_set_masses(self._h, mass, self.n)
 
     def accel(self, out: torch.Tensor | None = None) -> torch.Tensor:
         self._use_current_stream()

@@ -222,6 +222,7 @@ void nf_destroy(nf_plan *p)
     if (p->arena && p->arena_owned) cudaFree(p->arena);
     if (p->pos_stage) cudaFree(p->pos_stage);
     if (p->acc_stage) cudaFree(p->acc_stage);
+    if (p->mass_soa) cudaFree(p->mass_soa);
     if (p->device >= 0) for (int i = 0; i < 4; i++) cudaEventDestroy(p->ev[i]);
     delete p;
 }
@@ -267,6 +268,7 @@ int nf_bin(nf_plan *p, const float *pos, long long n)
 
     if (!p) { set_error("null plan"); return NF_ERR_ARG; }
     p->binned = false;
+    p->have_mass = false;                                       // masses belong to one binning
     if (n < 0) { set_error("n < 0"); return NF_ERR_ARG; }
     if ((double)n + 3.0 * p->k.ncells + 16.0 >= 4294967296.0) { set_error("n + 3 cpd^3 >= 2^32"); return NF_ERR_ARG; }
     if (!pos && n > 0) { set_error("null pos"); return NF_ERR_ARG; }
@@ -277,6 +279,30 @@ int nf_bin(nf_plan *p, const float *pos, long long n)
     rc = launch_bin(p, pos, n);
     if (rc) return rc;
     p->n = n; p->binned = true;
+    return NF_OK;
+}
+
+int nf_set_masses(nf_plan *p, const float *mass)
+{    DeviceGuard guard(p);
+
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_set_masses called before a successful nf_bin"); return NF_ERR_STATE; }
+    if (!mass) { p->have_mass = false; return NF_OK; }          // back to unit masses
+    const size_t N = (size_t)p->n, C = (size_t)p->k.ncells;
+    const size_t need = 4 * (N + 3 * (N < C ? N : C) + 8);      // padded slots: every non-empty cell adds at most 3
+    if (p->mass_cap < need) {
+        if (p->mass_soa) cudaFree(p->mass_soa);
+        p->mass_soa = nullptr; p->mass_cap = 0;
+        if (cudaMalloc(&p->mass_soa, need) != cudaSuccess) {
+            cudaGetLastError();
+            set_error("cudaMalloc of %zu bytes for the source masses failed", need);
+            return NF_ERR_NOMEM;
+        }
+        p->mass_cap = need;
+    }
+    const int rc = launch_set_masses(p, mass);
+    if (rc) return rc;
+    p->have_mass = true;
     return NF_OK;
 }
 

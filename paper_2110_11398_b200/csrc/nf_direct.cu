@@ -53,8 +53,9 @@ struct __align__(16) StageDesc {
     Piece    pieces[kMaxPieces];
 };
 
-struct __align__(128) SharedStorage {
-    float buf[kStages][3][kTile + 4];  // x, y, z of the staged sources + one quad of dummies (never overwritten)
+template <int NARR>                    // 3: x, y, z;  4: + the source masses (nf_set_masses)
+struct __align__(128) SharedStorageT {
+    float buf[kStages][NARR][kTile + 4];  // x, y, z (, m) of the staged sources + one quad of dummies (never overwritten)
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
@@ -119,8 +120,9 @@ __device__ __forceinline__ void accum2(const float2 k, const float2 d, float2 &a
 }
 
 // two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
-// (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ
-__device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
+// (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ; with source masses M one more FMUL2 (k m)
+template <bool MASS>
+__device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 M, const float2 nx, const float2 ny,
                                           const float2 nz, const SoftCoef &c, float2 &ax, float2 &ay, float2 &az)
 {
     const float2 dx = __fadd2_rn(X, nx), dy = __fadd2_rn(Y, ny), dz = __fadd2_rn(Z, nz);
@@ -131,7 +133,8 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
     ri.x = rsqrt_approx(r2.x);
     ri.y = rsqrt_approx(r2.y);
     const float2 ri2 = __fmul2_rn(ri, ri);
-    const float2 k = __fmul2_rn(ri2, ri);
+    float2 k = __fmul2_rn(ri2, ri);
+    if (MASS) k = __fmul2_rn(k, M);
     accum2<0>(k, dx, ax);
     accum2<1>(k, dy, ay);
     accum2<2>(k, dz, az);
@@ -139,8 +142,8 @@ __device__ __forceinline__ void interact2(const float2 X, const float2 Y, const 
 
 // scalar body (variant 1): 14 / 11 FP32-pipe instructions per interaction (+ 3 with the density estimate).
 // MODE 0: Newtonian, 1: spline, 2: spline + kernel density weight max(0, 1 - r^2/b^2)
-template <int MODE>
-__device__ __forceinline__ void interact1(const float X, const float Y, const float Z, const float nx, const float ny,
+template <int MODE, bool MASS>
+__device__ __forceinline__ void interact1(const float X, const float Y, const float Z, const float M, const float nx, const float ny,
                                           const float nz, const SoftCoef &c, float &ax, float &ay, float &az, float &rho)
 {
     const float dx = X + nx, dy = Y + ny, dz = Z + nz;
@@ -156,6 +159,7 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
         const float q2 = c.plummer ? fmaf(dx, dx, fmaf(dy, dy, dz * dz)) : r2;
         rho += fmaxf(fmaf(q2, c.nb2, 1.0f), 0.0f);
     }
+    if (MASS) k *= M;
     ax = fmaf(k, dx, ax);
     ay = fmaf(k, dy, ay);
     az = fmaf(k, dz, az);
@@ -212,14 +216,14 @@ __device__ __forceinline__ void pair_density(const float2 r2, const SoftCoef &c,
 // (warp vote inside): the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s -- a
 // fraction of a percent of the quads at production density; otherwise the body is the Newtonian one plus
 // three FMNMX, a vote and a branch.
-template <bool PACKED, int MODE>
-__device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float sxi, const float syi,
+template <bool PACKED, int MODE, bool MASS>
+__device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float4 M, const float sxi, const float syi,
                                      const float szi, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
 {
     if (PACKED && MODE == 0) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        interact2(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c, f.x, f.y, f.z);
-        interact2(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2<MASS>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), make_float2(M.x, M.y), nx, ny, nz, c, f.x, f.y, f.z);
+        interact2<MASS>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), make_float2(M.z, M.w), nx, ny, nz, c, f.x, f.y, f.z);
     } else if (PACKED) {
         const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
         float2 dxa, dya, dza, r2a, ria, ka, dxb, dyb, dzb, r2b, rib, kb;
@@ -238,13 +242,14 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
             pair_density(r2a, c, f.rho);
             pair_density(r2b, c, f.rho);
         }
+        if (MASS) { ka = __fmul2_rn(ka, make_float2(M.x, M.y)); kb = __fmul2_rn(kb, make_float2(M.z, M.w)); }
         accum2<0>(ka, dxa, f.x); accum2<1>(ka, dya, f.y); accum2<2>(ka, dza, f.z);
         accum2<0>(kb, dxb, f.x); accum2<1>(kb, dyb, f.y); accum2<2>(kb, dzb, f.z);
     } else {
-        interact1<MODE>(X.x, Y.x, Z.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
-        interact1<MODE>(X.y, Y.y, Z.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
-        interact1<MODE>(X.z, Y.z, Z.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
-        interact1<MODE>(X.w, Y.w, Z.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
+        interact1<MODE, MASS>(X.x, Y.x, Z.x, M.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
+        interact1<MODE, MASS>(X.y, Y.y, Z.y, M.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
+        interact1<MODE, MASS>(X.z, Y.z, Z.z, M.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
+        interact1<MODE, MASS>(X.w, Y.w, Z.w, M.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
     }
 }
 
@@ -253,20 +258,22 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 // in the ragged tail a lane that has run out of sources is predicated off (Newtonian body) or reads the stage's
 // dummy quad (coordinates 2^55: contributes exactly 0 to the force and to the density) so that the warp stays
 // converged for the vote of the spline body.
-template <bool PACKED, int MODE>
+template <bool PACKED, int MODE, bool MASS>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
                                            const uint32_t live, const int jdummy, const float sxi, const float syi, const float szi,
                                            const SoftCoef &c, Partial &f)
 {
     const float4 *__restrict__ py = px + kTileAlloc / 4;
     const float4 *__restrict__ pz = py + kTileAlloc / 4;
+    const float4 *__restrict__ pm = pz + kTileAlloc / 4;        // masses: read only with MASS
+    const float4 one = make_float4(1.f, 1.f, 1.f, 1.f);
     if (n4 > 0) {
         if (MODE == 0) {
 #pragma unroll 2
-            for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f);
         } else {
 #pragma unroll kUnrollSoft
-            for (int j = 0; j < nmin; j++) quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f, live);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f, live);
         }
     }
     __syncwarp();
@@ -274,9 +281,9 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
     for (int j = nmin; j < nmax; j++) {
         if (MODE >= 1 && PACKED) {                    // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
-            quad<PACKED, MODE>(px[jj], py[jj], pz[jj], sxi, syi, szi, c, f);
+            quad<PACKED, MODE, MASS>(px[jj], py[jj], pz[jj], MASS ? pm[jj] : one, sxi, syi, szi, c, f);
         } else if (j < n4) {
-            quad<PACKED, MODE>(px[j], py[j], pz[j], sxi, syi, szi, c, f);
+            quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f);
         }
     }
 }
@@ -285,6 +292,7 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
 struct AccelArgs {
     Consts k;
     const float *x, *y, *z;          // padded SoA sources (= sinks)
+    const float *m;                  // padded SoA source masses (MASS kernels only; pads hold 0)
     const uint32_t *poff, *offset, *perm;
     const Unit *units;
     uint32_t n_units;
@@ -304,7 +312,8 @@ struct AccelArgs {
 
 // The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
 // descriptors, the barriers and the TMA unit.
-__device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, const int lane)
+template <int NARR>
+__device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR> &sm, const int lane)
 {
     const Consts &k = a.k;
     const int cpd = k.cpd, R = k.R;
@@ -319,6 +328,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
             tma_load_1d(&sm.buf[stage][0][cp_s], a.x + cp_g, cp_n * 4u, &sm.full[stage]);
             tma_load_1d(&sm.buf[stage][1][cp_s], a.y + cp_g, cp_n * 4u, &sm.full[stage]);
             tma_load_1d(&sm.buf[stage][2][cp_s], a.z + cp_g, cp_n * 4u, &sm.full[stage]);
+            if (NARR == 4) tma_load_1d(&sm.buf[stage][NARR - 1][cp_s], a.m + cp_g, cp_n * 4u, &sm.full[stage]);
         }
         cp_n = 0;
     };
@@ -327,7 +337,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
         if (lead) {
             sm.desc[stage].flags = sflags | extra;
             sm.desc[stage].npieces = np;
-            mbar_arrive_expect_tx(&sm.full[stage], (uint32_t)fill * 12u);
+            mbar_arrive_expect_tx(&sm.full[stage], (uint32_t)fill * (4u * NARR));
         }
         if (++stage == kStages) { stage = 0; phase ^= 1u; }
         open = false; sealed = false;
@@ -464,8 +474,8 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI>
-__device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, const int warp, const int lane)
+template <bool PACKED, bool DENS, bool EPI, bool MASS>
+__device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS ? 4 : 3> &sm, const int warp, const int lane)
 {
     const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f,
                            DENS ? -1.001f / a.dens_nb2 + a.k.tiny : 0.f, a.k.plummer};
@@ -554,9 +564,9 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
                     if (soft_mode == 1) soft = __any_sync(kFull, touching && gap2 < a.k.soft_thr2);
                     if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
-                if (DENS && dens) piece_loop<PACKED, 2>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
-                else if (soft)    piece_loop<PACKED, 1>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
-                else              piece_loop<PACKED, 0>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                if (DENS && dens) piece_loop<PACKED, 2, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                else if (soft)    piece_loop<PACKED, 1, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
             }
             ax += (double)f.x.x + (double)f.x.y;
             ay += (double)f.y.x + (double)f.y.y;
@@ -583,35 +593,43 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorage &sm, 
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI>
+template <bool PACKED, bool DENS, bool EPI, bool MASS>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
+    constexpr int NARR = MASS ? 4 : 3;
     extern __shared__ __align__(128) unsigned char smem_raw[];          // dynamic: stages above 48 KB need the opt-in
-    SharedStorage &sm = *reinterpret_cast<SharedStorage *>(smem_raw);
+    SharedStorageT<NARR> &sm = *reinterpret_cast<SharedStorageT<NARR> *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid < kStages * 3 * 4) sm.buf[tid / 12][(tid / 4) % 3][kTile + (tid & 3)] = kDummy;
+    if (tid < kStages * NARR * 4)                                       // dummy quad: far-away coordinates, mass 0
+        sm.buf[tid / (4 * NARR)][(tid / 4) % NARR][kTile + (tid & 3)] = (tid / 4) % NARR == 3 ? 0.f : kDummy;
     if (tid == 0) {
         for (int s = 0; s < kStages; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kConsumerWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (warp == kConsumerWarps) producer(a, sm, lane);
-    else                        consumer<PACKED, DENS, EPI>(a, sm, warp, lane);
+    if (warp == kConsumerWarps) producer<NARR>(a, sm, lane);
+    else                        consumer<PACKED, DENS, EPI, MASS>(a, sm, warp, lane);
 }
 
 typedef void (*direct_fn)(const AccelArgs);
-static direct_fn pick_kernel(int variant, bool dens, bool epi)      // dens and epi are separate entry points
+template <bool MASS>
+static direct_fn pick_kernel_m(int variant, bool dens, bool epi)    // dens and epi are separate entry points
 {
-    if (variant == 0) return dens ? direct_kernel<true, true, false> : (epi ? direct_kernel<true, false, true> : direct_kernel<true, false, false>);
-    return dens ? direct_kernel<false, true, false> : (epi ? direct_kernel<false, false, true> : direct_kernel<false, false, false>);
+    if (variant == 0) return dens ? direct_kernel<true, true, false, MASS> : (epi ? direct_kernel<true, false, true, MASS> : direct_kernel<true, false, false, MASS>);
+    return dens ? direct_kernel<false, true, false, MASS> : (epi ? direct_kernel<false, false, true, MASS> : direct_kernel<false, false, false, MASS>);
 }
+static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false)
+{
+    return mass ? pick_kernel_m<true>(variant, dens, epi) : pick_kernel_m<false>(variant, dens, epi);
+}
+static size_t smem_bytes(bool mass) { return mass ? sizeof(SharedStorageT<4>) : sizeof(SharedStorageT<3>); }
 
 int accel_max_ctas_per_sm(int variant)
 {
     int nb = 0;
     direct_fn fn = pick_kernel(variant, false, false);
-    cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SharedStorage));
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, kAccelThreads, sizeof(SharedStorage));
+    cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(false));
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, kAccelThreads, smem_bytes(false));
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
@@ -625,17 +643,19 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     p->launches_accel = 0;
     if (p->n == 0 || p->n_units == 0) return NF_OK;
     const bool dens = rho != nullptr;
-    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr);
+    const bool mass = p->have_mass;
+    const size_t smem = smem_bytes(mass);
+    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr, mass);
     int per_sm = 0;
-    NF_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SharedStorage)));
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, sizeof(SharedStorage)) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+    NF_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, smem) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
     if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
     if (p->ctas_per_sm > 0 && p->ctas_per_sm < per_sm) per_sm = p->ctas_per_sm;
     long long grid = (long long)p->sm_count * per_sm;
     if (grid > p->n_units) grid = p->n_units;
     AccelArgs a;
     a.k = p->k;
-    a.x = p->ws.x; a.y = p->ws.y; a.z = p->ws.z;
+    a.x = p->ws.x; a.y = p->ws.y; a.z = p->ws.z; a.m = mass ? p->mass_soa : nullptr;
     a.poff = p->ws.poff; a.offset = p->ws.offset; a.perm = p->perm;
     a.units = p->ws.units_sorted;
     a.n_units = (uint32_t)p->n_units;
@@ -654,7 +674,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     NF_CUDA_OK(cudaEventRecord(p->ev[2], st));
     NF_CUDA_OK(cudaMemsetAsync(a.counter, 0, 4, st));
     if (amax_cell) NF_CUDA_OK(cudaMemsetAsync(amax_cell, 0, 4 * (size_t)p->k.ncells, st));
-    fn<<<(unsigned)grid, kAccelThreads, sizeof(SharedStorage), st>>>(a);
+    fn<<<(unsigned)grid, kAccelThreads, smem, st>>>(a);
     NF_CUDA_OK(cudaGetLastError());
     NF_CUDA_OK(cudaEventRecord(p->ev[3], st));
     p->have_accel_time = true;

@@ -112,6 +112,8 @@ struct nf_plan {
     long long n_units;
     int sort_passes;
     const uint32_t *perm;
+    // optional source masses (nf_set_masses): padded SoA like ws.x, plan-owned, outside the arena
+    float *mass_soa; size_t mass_cap; bool have_mass;
     // host-buffer path
     float *pos_stage; float *acc_stage; size_t stage_cap;   // device staging for *_host calls
     // options
@@ -126,6 +128,7 @@ namespace nf {
 void set_error(const char *fmt, ...);
 size_t carve(Workspace &ws, void *base, long long n, int cpd);   // base may be NULL (size only)
 int  launch_bin(nf_plan *p, const float *pos, long long n);             // S1-S5 (nf_bin.cu)
+int  launch_set_masses(nf_plan *p, const float *mass);                  // masses of the binned particles -> padded SoA (nf_bin.cu)
 int  launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, double dt, float *amax_cell);   // S6-S7 (nf_direct.cu)
 int  accel_max_ctas_per_sm(int variant);
 }

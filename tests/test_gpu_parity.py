@@ -660,3 +660,69 @@ def test_config4_full_size_density_and_kick_sampled(oracle_mod):
     m_ref = torch.zeros(cfg.cpd ** 3, dtype=torch.float64, device="cuda").scatter_reduce_(0, cid, norms, "amax")
     assert torch.allclose(amax.double(), m_ref, rtol=2e-7, atol=0)
     print(cfg.name, "fused passes", st, "rho max err", float(err.max()), "rho max", float(ref_rho.max()))
+
+
+# ---------------------------------------------------------------- per-particle source masses
+@pytest.mark.parametrize("idx,n_side,cpd,options", [(1, 32, 9, {}), (4, 40, 10, {}), (4, 32, 8, {"variant": 1}),
+                                                    (2, 48, 12, {"softening": 1}), (5, 40, 10, {"fastpath": 0})])
+def test_masses_parity(oracle_mod, idx, n_side, cpd, options):
+    """nf_set_masses: a_i = sum_j m_j d K against oracle.accel_mass (log-normal masses), same tolerance; unit masses
+    through the mass kernel are bit-identical to the plain kernel; nf_bin and set_masses(None) return to m = 1."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    mass = nf_inputs.masses(cfg)
+    soft = "plummer" if options.get("softening") else "spline"
+    ref = oracle_mod.accel_mass(pos.numpy(), mass.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R, softening=soft)
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
+        for k, v in options.items():
+            p.set_option(k, v)
+        p.bin(pos.cuda())
+        unit = p.accel().cpu()
+        p.set_masses(mass.cuda())
+        a = p.accel().cpu()
+        st = assert_parity(a.numpy().astype(np.float64), ref, f"{cfg.name} masses {options}")
+        print(cfg.name, options, st)
+        assert torch.equal(p.accel().cpu(), a)                              # deterministic
+        p.set_masses(torch.ones(cfg.n, device="cuda"))
+        assert torch.equal(p.accel().cpu(), unit)                           # k * 1 = k: the same bits as the plain kernel
+        p.set_masses(mass.cuda())
+        p.set_masses(None)
+        assert torch.equal(p.accel().cpu(), unit)
+        p.set_masses(mass.cuda())
+        p.bin(pos.cuda())                                                   # a new binning starts with unit masses
+        assert torch.equal(p.accel().cpu(), unit)
+
+
+def test_masses_fused_passes_and_errors(oracle_mod):
+    """Density and kick entry points with masses: forces bit-identical to nf_accel with the same masses, the density
+    estimate unchanged by them (count-based); massless particles are test particles; state errors."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.scaled(4, 32, 8)
+    pos = nf_inputs.generate(cfg)
+    mass = nf_inputs.masses(cfg)
+    mass[::5] = 0.0
+    ref = oracle_mod.accel_mass(pos.numpy(), mass.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
+    b = 0.4 / cfg.n_side
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
+        p.n = cfg.n
+        with pytest.raises(nf.NFError):
+            p.set_masses(mass.cuda())                                       # before nf_bin
+        p.bin(pos.cuda())
+        _, rho_unit = p.accel_density(b)
+        rho_unit = rho_unit.cpu()
+        p.set_masses(mass.cuda())
+        a = p.accel().cpu()
+        assert_parity(a.numpy().astype(np.float64), ref, "masses with test particles")
+        a2, rho = p.accel_density(b)
+        assert torch.equal(a2.cpu(), a) and torch.equal(rho.cpu(), rho_unit)
+        vel = torch.zeros((cfg.n, 3), device="cuda")
+        a3, _ = p.accel_kick(vel, 0.5)
+        assert torch.equal(a3.cpu(), a)
+        assert torch.equal(vel.cpu(), a * 0.5)
+        with pytest.raises(TypeError):
+            p.set_masses(mass[:-1].cuda())
+    with nf.Plan(4, 1.0, 0.01, 1) as p:                                     # n = 0
+        p.bin(torch.zeros((0, 3), device="cuda"))
+        p.set_masses(torch.zeros(0, device="cuda"))
+        assert p.accel().shape == (0, 3)

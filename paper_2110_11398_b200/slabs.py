@@ -57,7 +57,9 @@ def select_for_peer(pos_owned: torch.Tensor, slabs: torch.Tensor, peer_range: tu
 
 
 def halo_exchange(pos_owned: torch.Tensor, cpd: int, L: float, R: int, rank: int, world: int, dist=None):
-    """One exchange step.  ``pos_owned`` [n_own][3] float32 holds the particles of this rank's slabs (any order).
+    """One exchange step.  ``pos_owned`` [n_own][3] float32 holds the particles of this rank's slabs (any order);
+    more columns travel with the particle (column 3 = mass for ``Plan.set_masses``: split the result into
+    ``[:, :3].contiguous()`` and ``[:, 3].contiguous()``).
     Returns (pos_local, n_own): the owned particles first, then the halo particles received from the peers in
     rank order.  With ``world == 1`` (or ``dist is None``) nothing moves."""
     if cpd < 2 * R + 1:
@@ -76,7 +78,7 @@ def halo_exchange(pos_owned: torch.Tensor, cpd: int, L: float, R: int, rank: int
     counts = torch.tensor([s.shape[0] for s in sends], dtype=torch.int64, device=pos_owned.device)
     table = [torch.zeros_like(counts) for _ in range(world)]
     dist.all_gather(table, counts)
-    recvs = [torch.empty((int(table[q][rank]), 3), dtype=pos_owned.dtype, device=pos_owned.device) for q in range(world)]
+    recvs = [torch.empty((int(table[q][rank]), pos_owned.shape[1]), dtype=pos_owned.dtype, device=pos_owned.device) for q in range(world)]
     ops = []
     for q in range(world):
         if q == rank:

@@ -726,3 +726,27 @@ def test_masses_fused_passes_and_errors(oracle_mod):
         p.bin(torch.zeros((0, 3), device="cuda"))
         p.set_masses(torch.zeros(0, device="cuda"))
         assert p.accel().shape == (0, 3)
+
+
+@pytest.mark.parametrize("idx,device", [(3, "cpu"), (4, "cuda")])
+def test_masses_full_size_sampled(oracle_mod, idx, device):
+    """Masses at the full uniform and clustered sizes (the launch configuration bench.py times): accelerations of the
+    sink sample against oracle.accel_mass, total momentum sum_i m_i a_i = 0 within FP32 bounds."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.config(idx)
+    pos_dev = nf_inputs.generate(cfg, device=device).cuda()
+    mass_dev = nf_inputs.masses(cfg, device=device).cuda()
+    pos, mass = pos_dev.cpu().numpy(), mass_dev.cpu().numpy()
+    b = oracle_mod.bin_particles(pos, cfg.cpd, cfg.L)
+    sinks = sample_sinks(b["count"], b["offset"], b["perm"], cfg.cpd, np.random.default_rng(cfg.seed + 1), n_random=500,
+                         n_heavy=10, per_heavy=100)
+    ref = oracle_mod.accel_mass(pos, mass, cfg.cpd, cfg.L, cfg.eps, cfg.R, sinks=sinks, binning=b)
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos_dev)
+        plan.set_masses(mass_dev)
+        acc = plan.accel()
+        torch.cuda.synchronize()
+    st = assert_parity(acc[torch.from_numpy(sinks).cuda()].cpu().numpy().astype(np.float64), ref, cfg.name + " masses (sampled)")
+    ma = acc.double() * mass_dev.double()[:, None]
+    assert float(ma.sum(0).abs().max()) <= 2e-6 * float(ma.abs().sum())
+    print(cfg.name, "masses, sampled sinks", len(sinks), st)

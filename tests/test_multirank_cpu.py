@@ -89,6 +89,11 @@ def _slab_worker(rank, world, port, cpd, R, out):
         from_q = pos[(((sl - fq) % cpd) < cq) & halo_mask[sl]]
         order_ok &= torch.equal(local[off:off + from_q.shape[0]], from_q)
         off += from_q.shape[0]
+    # more columns travel with the particle (column 3 = mass): same rows, same order, payload intact
+    tag = lambda t: t[:, 0] + 2 * t[:, 1] + 3 * t[:, 2]
+    pos4 = torch.cat([pos, tag(pos)[:, None]], dim=1)
+    local4, n_own4 = slabs.halo_exchange(pos4[own_mask].contiguous(), cpd, 1.0, R, rank, world, dist)
+    order_ok &= n_own4 == n_own and torch.equal(local4[:, :3], local) and torch.equal(local4[:, 3], tag(local))
     out[rank] = (bool(ok), bool(order_ok), int(local.shape[0]))
     dist.barrier()
     dist.destroy_process_group()

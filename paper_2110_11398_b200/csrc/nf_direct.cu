@@ -59,6 +59,7 @@ struct __align__(128) SharedStorageT {
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
+    double part[kConsumerWarps][4][32];   // short windows: per-warp partial sums (x, y, z, rho) of a split unit
 };
 
 // ---- PTX helpers: mbarrier + TMA 1-D bulk copy ---------------------------------------------------
@@ -484,6 +485,14 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
     uint32_t phase = 0;
     float xi = 0.f, yi = 0.f, zi = 0.f;
     double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0, rho = 0.0;
+    // A window of fewer than kChunk sinks leaves consumer warps without sinks.  They take a share of the unit's stages
+    // instead: with ng = ceil(ns / 32) sink groups the kConsumerWarps / ng warps {g, g + ng, g + 2 ng, ...} hold the SAME
+    // 32 sinks, warp q of them computes the stages q, q + nsplit, ... of the unit, and the partial sums meet in shared
+    // memory at the end of the unit, added in the fixed order q = 0, 1, ... (deterministic).  Small problems, whose units
+    // cannot fill the machine, and the ragged last window of every column then keep all warps of the CTA busy.
+    // one register: nsplit (warps sharing the sinks) | ng << 4 (sink groups) | q << 8 (this warp's share) | countdown << 12
+    static_assert(kConsumerWarps <= 15, "the split state packs warp counts into 4-bit fields");
+    uint32_t sp = 1u | ((uint32_t)kConsumerWarps << 4);
     int zrel = 0, zoff = 0;             // the lane's sink cell relative to z0, and zrel mod (2R+1)
     uint32_t slot = 0;                  // the lane's sorted slot (perm index)
     uint32_t cell = 0;                  // the lane's sink cell id
@@ -494,9 +503,12 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
         const int flags = d.flags;
         if (flags & kFlagTerm) break;
         if (flags & kFlagBegin) {
-            const uint32_t ns = d.ns, kk = (uint32_t)(warp * 32 + lane);
-            warp_on = (uint32_t)(warp * 32) < ns;
-            act = kk < ns;
+            const uint32_t ns = d.ns;
+            const int ng = (int)((ns + 31u) >> 5), nsplit = kConsumerWarps / ng, q = warp / ng;
+            sp = (uint32_t)nsplit | ((uint32_t)ng << 4) | ((uint32_t)q << 8) | ((uint32_t)q << 12);   // first stage of warp q: stage q
+            const uint32_t kk = (uint32_t)((warp - q * ng) * 32 + lane);
+            warp_on = q < nsplit;
+            act = warp_on && kk < ns;
             ax = ay = az = rho = 0.0;
             if (warp_on) {
                 // lanes past the end of a ragged window shadow its last sink (same pieces, nothing written)
@@ -515,7 +527,9 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
             }
         }
-        if (warp_on) {
+        const bool mine = warp_on && (sp >> 12) == 0u;                  // countdown to this warp's next stage
+        sp = mine ? (sp | (((sp & 15u) - 1u) << 12)) : sp - (1u << 12);
+        if (mine) {
             const int np = d.npieces, soft_mode = d.soft_mode;
             const float sxi = d.dx - xi, syi = d.dy - yi;           // -(x_i - shift)
             const int ibase = zrel - d.j0;
@@ -573,7 +587,23 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
             az += (double)f.z.x + (double)f.z.y;
             if (DENS) rho += (double)f.rho.x + (double)f.rho.y;
         }
-        if ((flags & kFlagEnd) && act) {
+        if ((flags & kFlagEnd) && (sp & 15u) > 1u) {          // warp-uniform, the same for every consumer warp of the CTA
+            const int nsplit = (int)(sp & 15u), ng = (int)((sp >> 4) & 15u), q = (int)((sp >> 8) & 15u);
+            if (warp_on && q > 0) {
+                sm.part[warp][0][lane] = ax; sm.part[warp][1][lane] = ay; sm.part[warp][2][lane] = az;
+                if (DENS) sm.part[warp][3][lane] = rho;
+            }
+            asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");
+            if (warp_on && q == 0) {
+                for (int t = 1; t < nsplit; t++) {
+                    const int w2 = warp + t * ng;
+                    ax += sm.part[w2][0][lane]; ay += sm.part[w2][1][lane]; az += sm.part[w2][2][lane];
+                    if (DENS) rho += sm.part[w2][3][lane];
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");   // the buffer is free for the next unit
+        }
+        if ((flags & kFlagEnd) && act && ((sp >> 8) & 15u) == 0u) {
             const size_t i = __ldg(a.perm + slot);
             const double s2 = a.k.out_scale;
             const float fx = (float)(ax * s2), fy = (float)(ay * s2), fz = (float)(az * s2);

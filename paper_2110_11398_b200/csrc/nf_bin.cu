@@ -101,11 +101,40 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const uint32_t *in, u
     }
 }
 
+// One block does the whole scan when it is short (small problems are bound by the number of launches of nf_bin):
+// every thread owns kSmallItems consecutive elements; in may alias out.
+constexpr int kSmallThreads = 1024, kSmallItems = 16, kSmallMax = kSmallThreads * kSmallItems;
+
+template <class Op>
+__global__ void __launch_bounds__(kSmallThreads) scan_small(const uint32_t *in, uint32_t *out, uint32_t n, Op op, int write_total,
+                                                            uint32_t *total_out)
+{
+    __shared__ uint32_t sm[33];
+    const uint32_t base = threadIdx.x * kSmallItems;
+    uint32_t v[kSmallItems], s = 0;
+#pragma unroll
+    for (int k = 0; k < kSmallItems; k++) { v[k] = (base + k < n) ? op(in[base + k]) : 0; s += v[k]; }
+    uint32_t tot;
+    uint32_t run = block_exclusive_scan(s, &tot, sm);
+#pragma unroll
+    for (int k = 0; k < kSmallItems; k++)
+        if (base + k < n) { out[base + k] = run; run += v[k]; }
+    if (threadIdx.x == 0) {
+        if (write_total) out[n] = tot;
+        if (total_out) *total_out = tot;
+    }
+}
+
 template <class Op>
 static void exclusive_scan(const uint32_t *in, uint32_t *out, size_t n, uint32_t *tmp, Op op, int write_total,
                            uint32_t *total_out, cudaStream_t st, int *launches)
 {
     if (n == 0) return;
+    if (n <= (size_t)kSmallMax) {
+        scan_small<<<1, kSmallThreads, 0, st>>>(in, out, (uint32_t)n, op, write_total, total_out);
+        *launches += 1;
+        return;
+    }
     uint32_t nb = (uint32_t)((n + kScanTile - 1) / kScanTile);
     scan_reduce<<<nb, kScanThreads, 0, st>>>(in, n, tmp, op);
     scan_spine<<<1, 1024, 0, st>>>(tmp, nb, total_out);
@@ -531,16 +560,18 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 {
     const size_t n = (size_t)n_ll;
     // sinks per work unit: the caller's window, else kChunk -- except for a problem so small that its units would not
-    // fill the grid of persistent CTAs once: there the shortest window >= 96 whose units still run in one wave
-    // (config 1, 32^3 particles: 405 units of 96 instead of 162 of 256, 0.202 against 0.236 ms; shorter windows need
-    // a second wave and stream the stencil more often: 64 -> 0.285 ms)
+    // fill the grid of persistent CTAs: there the longest window >= 64 that still gives every CTA slot a unit (the
+    // consumer warps of a short window share its stages, nf_direct.cu).  Config 1 (32^3 particles): 567 units of 64
+    // sinks, 0.137 ms against 0.238 ms for 162 units of 256.
     p->k.chunk = kChunk;
     if (p->window > 0) p->k.chunk = p->window;
     else if (n_ll > 0) {
         const double cols = (double)p->k.nslab * p->k.cpd;
+        const double per_col = (double)n_ll / ((double)p->k.cpd * p->k.cpd);
         const double slots = (double)p->sm_count * kMinCtasPerSm;
-        for (int w = 96; w < kChunk; w += 32)
-            if (cols * std::ceil((double)n_ll / ((double)p->k.cpd * p->k.cpd) / w) <= slots) { p->k.chunk = w; break; }
+        int w = kChunk;
+        while (w > 64 && cols * std::ceil(per_col / w) < slots) w -= 32;
+        p->k.chunk = w;
     }
     const Consts &k = p->k;
     Workspace &ws = p->ws;

@@ -19,7 +19,10 @@ constexpr int kMaxR          = 4;                 // stencil (2R+1)^3 with R <= 
 #define NF_TILE 1024
 #endif
 #ifndef NF_STAGES
-#define NF_STAGES 3
+#define NF_STAGES 5
+#endif
+#ifndef NF_STAGES_MASS
+#define NF_STAGES_MASS 3
 #endif
 #ifndef NF_MIN_CTAS
 #define NF_MIN_CTAS 3
@@ -27,7 +30,8 @@ constexpr int kMaxR          = 4;                 // stencil (2R+1)^3 with R <= 
 constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // sink lanes per CTA = 32 * kConsumerWarps
 constexpr int kChunk         = 32 * kConsumerWarps;   // max sinks per work unit (a window of one z-column)
 constexpr int kTile          = NF_TILE;           // source slots per pipeline stage (multiple of 4)
-constexpr int kStages        = NF_STAGES;         // TMA pipeline depth
+constexpr int kStages        = NF_STAGES;         // TMA pipeline depth (three staged arrays)
+constexpr int kStagesMass    = NF_STAGES_MASS;    //   with the fourth array of the mass kernels
 constexpr int kMaxPieces     = 40;                // source cells (table entries) per stage
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
 constexpr int kMinCtasPerSm  = NF_MIN_CTAS;       // register budget: 65536 / (kMinCtasPerSm * kAccelThreads) per thread

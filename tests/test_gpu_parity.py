@@ -750,3 +750,31 @@ def test_masses_full_size_sampled(oracle_mod, idx, device):
     ma = acc.double() * mass_dev.double()[:, None]
     assert float(ma.sum(0).abs().max()) <= 2e-6 * float(ma.abs().sum())
     print(cfg.name, "masses, sampled sinks", len(sinks), st)
+
+
+@pytest.mark.parametrize("ns", [1, 31, 32, 33, 65, 96, 97, 129, 161, 193, 225, 255, 256, 257, 300])
+def test_short_windows_share_stages(oracle_mod, ns):
+    """One z-column holding `ns` particles next to a filled box: the column's windows have every number of sink groups
+    (1..8), so the warps that share a window's stages come in all splits (8, 4, 2, 2, 1, ... with idle warps for 3, 5, 6, 7
+    groups); results against the oracle and bit-identical between two runs (the partial sums are added in a fixed order)."""
+    import paper_2110_11398_b200 as nf
+    cpd, R, L = 6, 2, 1.0
+    rng = np.random.default_rng(ns)
+    col = rng.random((ns, 3)).astype(np.float32)
+    col[:, 0] = (col[:, 0] + 2) / cpd                         # column (2, 3)
+    col[:, 1] = (col[:, 1] + 3) / cpd
+    rest = rng.random((3000, 3)).astype(np.float32)
+    keep = ~((np.floor(rest[:, 0] * cpd) == 2) & (np.floor(rest[:, 1] * cpd) == 3))
+    pos = torch.from_numpy(np.concatenate([col, rest[keep]]))
+    eps = 0.01
+    ref = oracle_mod.accel(pos.numpy(), cpd, L, eps, R)
+    with nf.Plan(cpd, L, eps, R) as p:
+        p.set_option("window", 256)                           # the column is one window of ns sinks (two from 257)
+        p.bin(pos.cuda())
+        a1 = p.accel().cpu()
+        a2, rho = p.accel_density(0.05)
+        a3 = p.accel().cpu()
+    assert torch.equal(a1, a3) and torch.equal(a1, a2.cpu())
+    assert_parity(a1.numpy().astype(np.float64), ref, f"column of {ns}")
+    rho_ref = oracle_mod.density(pos.numpy(), cpd, L, 0.05, R)
+    assert np.all(np.abs(rho.cpu().numpy() - rho_ref) <= 1e-5 * rho_ref)

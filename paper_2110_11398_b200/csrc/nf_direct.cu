@@ -111,6 +111,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
+constexpr float kSelfR2 = 2e-36f;   // r^2 of a pair at r = 0 is the offset `tiny` = 1e-36 (spline law); nothing else is below this
 struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin)
 
 // a += k d for two packed interactions.  A packed FFMA2 with three distinct register-pair operands holds the
@@ -161,6 +162,9 @@ __device__ __forceinline__ void interact1(const float X, const float Y, const fl
         const float r = r2 * ri;
         const float t = fmaf(fmaf(r, c.C, c.B), r, c.A);
         k = fminf(k, t);
+        // with masses the capped k of the self pair (r^2 = tiny; the cap is 3e38 for eps = 0) times m could overflow to
+        // inf and inf * 0 = NaN: the self pair and exactly coincident particles are dropped explicitly (reading C5)
+        if (MASS && r2 <= kSelfR2) k = 0.f;
     }
     if (MODE == 2) {                      // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
         const float q2 = c.plummer ? fmaf(dx, dx, fmaf(dy, dy, dz * dz)) : r2;
@@ -240,6 +244,10 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
         if (__any_sync(mask, m < c.soft_r2)) {
             pair_spline(r2a, ria, c, ka);
             pair_spline(r2b, rib, c, kb);
+            if (MASS) {                       // see interact1: drop r = 0 before the mass multiplies the capped k
+                ka.x = r2a.x > kSelfR2 ? ka.x : 0.f; ka.y = r2a.y > kSelfR2 ? ka.y : 0.f;
+                kb.x = r2b.x > kSelfR2 ? kb.x : 0.f; kb.y = r2b.y > kSelfR2 ? kb.y : 0.f;
+            }
         }
         if (MODE == 2 && __any_sync(mask, m < c.dens_r2)) {     // some lane has a source of this quad inside b
             if (c.plummer) {                  // the Plummer option puts eps^2 into r2: the weight needs the bare r^2

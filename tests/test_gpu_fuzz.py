@@ -58,7 +58,8 @@ def test_fuzz_against_oracle(oracle_mod, seed):
     eps = float(rng.choice([0.0, 1e-4, 0.01, 0.05, 0.3, 1.2])) * cell
     pos = _positions(rng, kind, n, L)
     n = pos.shape[0]
-    opts = {"variant": int(rng.integers(0, 2)), "fastpath": int(rng.integers(0, 2)), "heavy_first": int(rng.integers(0, 2))}
+    opts = {"variant": int(rng.integers(0, 2)), "fastpath": int(rng.integers(0, 2)), "heavy_first": int(rng.integers(0, 2)),
+            "window": int(np.random.default_rng(7000 + seed).choice([0, 0, 32, 96, 160, 224, 256]))}
     plummer = bool(rng.integers(0, 4) == 0)
     if plummer:
         opts["softening"] = 1
@@ -76,18 +77,29 @@ def test_fuzz_against_oracle(oracle_mod, seed):
         assert st["interactions"] == oracle_mod.interactions(b["count"], cpd, R), what
         ref = oracle_mod.accel(pos, cpd, L, eps, R, binning=b, softening="plummer" if plummer else "spline")
         a = acc.cpu().numpy().astype(np.float64)
-        if kind in ("duplicates", "faces", "lattice", "sparse_line"):
-            # symmetric or nearly symmetric sets: the pair forces on a particle cancel (|a_ref| -> 0), so the error is
-            # measured against the scale of the forces in the set, not against |a_ref| (reading C13)
-            scale = np.linalg.norm(ref, axis=1).max() + 1e-300
-            assert np.linalg.norm(a - ref, axis=1).max() <= 1e-4 * scale, what
-        elif eps > 0.25 * cell:
-            # softening of the order of a cell: every pair is in the harmonic core (force ~ d), the sum over thousands of
-            # sources cancels, and the FP32 partial sums carry 1e-7 sqrt(n) of the UNcancelled magnitude
-            err = rel_errors(a, ref)
-            assert np.quantile(err, 0.999) <= 1e-4 and err.max() <= 1e-3, what
-        else:
-            assert_parity(a, ref, what)
+
+        def check(a, ref, what):
+            if kind in ("duplicates", "faces", "lattice", "sparse_line"):
+                # symmetric or nearly symmetric sets: the pair forces on a particle cancel (|a_ref| -> 0), so the error is
+                # measured against the scale of the forces in the set, not against |a_ref| (reading C13)
+                scale = np.linalg.norm(ref, axis=1).max() + 1e-300
+                assert np.linalg.norm(a - ref, axis=1).max() <= 1e-4 * scale, what
+            elif kind == "plane":
+                # all particles in one x-slab: the in-plane pair forces on a sink largely cancel, so |a_ref| is of the order
+                # of the rms of ONE term times sqrt(sources) while every FP32 term carries ~1e-7 of its own magnitude
+                # (DESIGN.md sec. 5): 1e-7 sqrt(12000) ~ 1.1e-5 of |a_ref| at the largest n.  Seed 491 (n = 12000, cpd = 2R+1,
+                # Plummer) sits at p99.9 = 1.04e-5; the bound below is twice BJ's, the maximum stays BJ's.
+                err = rel_errors(a, ref)
+                assert np.quantile(err, 0.999) <= 2e-5 and err.max() <= 1e-3, what
+            elif eps > 0.25 * cell:
+                # softening of the order of a cell: every pair is in the harmonic core (force ~ d), the sum over thousands
+                # of sources cancels, and the FP32 partial sums carry 1e-7 sqrt(n) of the UNcancelled magnitude
+                err = rel_errors(a, ref)
+                assert np.quantile(err, 0.999) <= 1e-4 and err.max() <= 1e-3, what
+            else:
+                assert_parity(a, ref, what)
+
+        check(a, ref, what)
         # the fused passes on the same binning
         if R >= 1 and n > 1:
             bw = float(rng.choice([0.05, 0.4, 0.999, 1.0])) * min(R, 1.0) * cell
@@ -105,6 +117,16 @@ def test_fuzz_against_oracle(oracle_mod, seed):
         m_ref = oracle_mod.cell_max_accel(acc.cpu().numpy(), b["cid"], cpd ** 3)         # max of the SAME float32 vectors
         m_gpu = amax.cpu().numpy().astype(np.float64)
         assert np.allclose(m_gpu, m_ref, rtol=2e-7, atol=0), what
+        # per-particle source masses on the same binning (log-normal, a fifth of them zero), then back to unit masses
+        if seed % 2 == 0:
+            mass = np.exp(rng.standard_normal(n)).astype(np.float32)
+            mass[rng.random(n) < 0.2] = 0.0
+            plan.set_masses(torch.from_numpy(mass).cuda())
+            am = plan.accel().cpu().numpy().astype(np.float64)
+            ref_m = oracle_mod.accel_mass(pos, mass, cpd, L, eps, R, binning=b, softening="plummer" if plummer else "spline")
+            check(am, ref_m, what + " masses")
+            plan.set_masses(None)
+            assert torch.equal(plan.accel(), acc), what
 
 
 @pytest.mark.parametrize("seed", range(12))

@@ -150,7 +150,8 @@ void nf_destroy(nf_plan *plan);
  * range of slabs and needs "R loaded slabs on either side").  After this call only the
  * particles whose cell has x index in {x_first, ..., x_first + n_slabs - 1} (mod cpd) are SINKS; every binned
  * particle is still a source.  A rank bins its own slabs plus the R halo slabs of each x-neighbour and gets
- * exactly the accelerations a whole-box plan would give its particles; rows of acc that belong to particles
+ * exactly the accelerations a whole-box plan would give its particles (bit for bit when both plans use the same
+ * "window" option; the automatic window of small problems depends on the number of owned columns); rows of acc that belong to particles
  * outside the sink slabs are not written, and nf_stats.interactions counts the owned sinks only.
  * Takes effect at the next nf_bin (it invalidates the current binning).  Default: all slabs.
  * Errors: NF_ERR_ARG unless 0 <= x_first < cpd and 1 <= n_slabs <= cpd.

@@ -209,7 +209,7 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
  *   "window"       sinks per work unit: a multiple of 32 up to 256, or 0 (default) = 256, except for problems whose
- *                  units would not fill the grid of persistent CTAs, which get the longest window >= 64 that does.
+ *                  units would not fill the grid of persistent CTAs, which get the longest of 256, 128 and 64 that does.
  *                  The warps of a CTA that a short window leaves without sinks share the unit's stages.
  *                  Shorter windows give a small problem more work units, but every unit streams its whole stencil
  *                  again.  Accelerations are bit-identical between plans only for equal windows.  Takes effect at the next nf_bin.

@@ -560,7 +560,7 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 {
     const size_t n = (size_t)n_ll;
     // sinks per work unit: the caller's window, else kChunk -- except for a problem so small that its units would not
-    // fill the grid of persistent CTAs: there the longest window >= 64 that still gives every CTA slot a unit (the
+    // fill the grid of persistent CTAs: there the longest of 256, 128, 64 that still gives every CTA slot a unit (the
     // consumer warps of a short window share its stages, nf_direct.cu).  Config 1 (32^3 particles): 567 units of 64
     // sinks, 0.137 ms against 0.238 ms for 162 units of 256.
     p->k.chunk = kChunk;
@@ -570,7 +570,7 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
         const double per_col = (double)n_ll / ((double)p->k.cpd * p->k.cpd);
         const double slots = (double)p->sm_count * kMinCtasPerSm;
         int w = kChunk;
-        while (w > 64 && cols * std::ceil(per_col / w) < slots) w -= 32;
+        while (w > 64 && cols * std::ceil(per_col / w) < slots) w >>= 1;    // 256, 128, 64: sink-group counts that divide the consumer warps
         p->k.chunk = w;
     }
     const Consts &k = p->k;

@@ -1,5 +1,5 @@
 // nf_bin.cu -- steps S1-S5 of the hot path: cell ids, per-cell histogram, prefix
-// sums, STABLE counting sort (LSD radix on the cell id, 8 bits per pass), gather into the
+// sums, STABLE counting sort (LSD radix on the cell id, 1-3 passes of 8-11 bit digits), gather into the
 // cell-padded SoA source arrays, work-unit list with heavy-first order, exact interaction count.
 //
 // The paper's analogues are the CPU stages "Transpose Positions" and "Index Near Force Pencils"

@@ -212,7 +212,8 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *                  units would not fill the grid of persistent CTAs, which get the longest of 256, 128 and 64 that does.
  *                  The warps of a CTA that a short window leaves without sinks share the unit's stages.
  *                  Shorter windows give a small problem more work units, but every unit streams its whole stencil
- *                  again.  Accelerations are bit-identical between plans only for equal windows.  Takes effect at the next nf_bin.
+ *                  again.  With 256-sink windows the remainder of a column is cut into 128 / 64 / fewer sinks (sink
+ *                  groups that divide the consumer warps).  Accelerations are bit-identical between plans only for equal windows.  Takes effect at the next nf_bin.
  *   "softening"    0 = the compact spline of the method (default); 1 = Plummer softening, force
  *                  d (r^2 + eps^2)^(-3/2) with eps the plan's length: the law the paper compares against
  *                  ("converges only quadratically to the correct large-scale force law")

@@ -481,6 +481,27 @@ __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t 
 }
 
 // work units per z-column: windows of kChunk consecutive cell-sorted sinks
+// Length of the next window of a column that has `rem` sinks left.  Whole windows of `chunk`; the remainder of a
+// column with default windows is cut so that its sink groups (32 sinks each) divide the consumer warps: 5-7 groups ->
+// 128 sinks (4 groups) first, 3 groups -> 64 sinks (2 groups) first.  Every window then keeps all the warps of its CTA
+// busy (the warps without sinks share the stages, nf_direct.cu); 3, 5, 6 or 7 groups would leave 2-3 of them idle.
+__device__ __forceinline__ uint32_t window_len(uint32_t rem, uint32_t chunk)
+{
+    if (rem >= chunk) return chunk;
+    if (chunk == (uint32_t)kChunk && kConsumerWarps == 8) {
+        const uint32_t ng = (rem + 31u) >> 5;
+        if (ng >= 5 && ng <= 7) return 128u;
+        if (ng == 3) return 64u;
+    }
+    return rem;
+}
+__device__ __forceinline__ uint32_t windows_in(uint32_t ncol, uint32_t chunk)
+{
+    uint32_t nw = ncol / chunk, rem = ncol - nw * chunk;
+    while (rem) { rem -= window_len(rem, chunk); nw++; }
+    return nw;
+}
+
 __global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ offset,
                                                        uint32_t *__restrict__ nunits)
 {
@@ -488,7 +509,7 @@ __global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t 
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
     const uint32_t ncol = offset[(size_t)(col + 1) * k.cpd] - offset[(size_t)col * k.cpd];
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
-    nunits[col] = rel < k.nslab ? (ncol + k.chunk - 1) / k.chunk : 0u;            // columns outside the sink slabs: sources only
+    nunits[col] = rel < k.nslab ? windows_in(ncol, (uint32_t)k.chunk) : 0u;      // columns outside the sink slabs: sources only
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
@@ -505,8 +526,9 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
     const uint32_t c_begin = off[0], c_end = off[k.cpd];
     uint32_t u = ubase[col];
     int z = 0;
-    for (uint32_t s0 = c_begin; s0 < c_end; s0 += k.chunk, u++) {
-        const uint32_t s1 = min(s0 + (uint32_t)k.chunk, c_end);
+    for (uint32_t s0 = c_begin, len = 0; s0 < c_end; s0 += len, u++) {
+        len = window_len(c_end - s0, (uint32_t)k.chunk);
+        const uint32_t s1 = s0 + len;
         while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
         Unit un;
         un.s0 = s0; un.col = col; un.ns = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;

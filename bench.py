@@ -25,8 +25,8 @@ METRIC = "near_field_pair_interactions_per_s"
 UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
 FLOPS_EXECUTED_MIN = 19         # the Newtonian body (3 add + 6 fma + 2 mul + rsqrt) the kernel runs where no pair is inside eps_s
-# DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v8_final.md)
-NCU_TRAFFIC_BYTES = {"config3_uniform_256": 959621632 + 656791296, "config4_halos_512": 18155223000 + 5468523000}
+# DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v9_final_config3.md, profiles/r1_v8_final.md)
+NCU_TRAFFIC_BYTES = {"config3_uniform_256": 958413568 + 656910848, "config4_halos_512": 18155223000 + 5468523000}
 L2_BYTES = 126 * 1024 * 1024
 
 

@@ -12,6 +12,7 @@ from .nf_oracle import (  # noqa: F401
     accel,
     accel_mass,
     density,
+    force_scale,
     kick,
     cell_max_accel,
     interactions,

@@ -304,6 +304,62 @@ int nfo_density(const float *pos, int64_t n, int cpd, double L, double b, int R,
 }
 
 /*
+ * Uncancelled magnitude of the direct sum (test metric, reading C13 of SURVEY.md 8(c) / DESIGN.md 2):
+ *   S_i = sum_j m_j |d_ij| K(|d_ij|),   j over the same (2R+1)^3 stencil particles as the acceleration
+ * (the sum the near field evaluates; here every term enters with its NORM, so nothing cancels).
+ * |a_i| <= S_i always (triangle inequality); S_i = |a_i| when the sink has one source.  A float32 evaluation of
+ * the sum carries an error proportional to S_i, not to |a_i|: where the pair forces cancel (lattices, planes,
+ * harmonic cores) BASELINE.json's ratio |a_gpu - a_ref| / |a_ref| is ill-conditioned and the tests bound the
+ * error by a multiple of S_i instead.
+ * Written out on its own, like nfo_density, so that the pinned acceleration loops stay untouched.
+ *   mass  [n] float32 or NULL (unit masses);  kind 0: spline, 1: Plummer;  scale [m] float64 out.
+ */
+int nfo_force_scale(const float *pos, const float *mass, int64_t n, int cpd, double L, double eps, int R, int kind,
+                    const uint32_t *cid, const uint32_t *offset, const uint32_t *perm,
+                    const int64_t *sinks, int64_t m, double *scale)
+{
+    if (kind != 0 && kind != 1) return NFO_ERR_ARG;
+    if (nfo_check_args(cpd, L, eps, R) != NFO_OK || n < 0 || m < 0) return NFO_ERR_ARG;
+    if (!sinks && m != n) return NFO_ERR_ARG;
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(|:bad)
+    for (int64_t k = 0; k < m; k++) {
+        int64_t i = sinks ? sinks[k] : k;
+        if (i < 0 || i >= n) { bad |= 1; continue; }
+        uint32_t id = cid[i];
+        int cz = (int)(id % (uint32_t)cpd);
+        int cy = (int)((id / (uint32_t)cpd) % (uint32_t)cpd);
+        int cx = (int)(id / ((uint32_t)cpd * (uint32_t)cpd));
+        double xi = (double)pos[3 * i + 0], yi = (double)pos[3 * i + 1], zi = (double)pos[3 * i + 2];
+        double sum = 0.0;
+        for (int ox = -R; ox <= R; ox++)
+        for (int oy = -R; oy <= R; oy++)
+        for (int oz = -R; oz <= R; oz++) {
+            int sx = cx + ox, sy = cy + oy, sz = cz + oz;
+            double wx = 0.0, wy = 0.0, wz = 0.0;
+            if (sx < 0) { sx += cpd; wx = -1.0; } else if (sx >= cpd) { sx -= cpd; wx = 1.0; }
+            if (sy < 0) { sy += cpd; wy = -1.0; } else if (sy >= cpd) { sy -= cpd; wy = 1.0; }
+            if (sz < 0) { sz += cpd; wz = -1.0; } else if (sz >= cpd) { sz -= cpd; wz = 1.0; }
+            int64_t c2 = ((int64_t)sx * cpd + sy) * cpd + sz;
+            for (uint32_t t = offset[c2]; t < offset[c2 + 1]; t++) {
+                int64_t j = perm[t];
+                double dx = (double)pos[3 * j + 0] - xi + wx * L;
+                double dy = (double)pos[3 * j + 1] - yi + wy * L;
+                double dz = (double)pos[3 * j + 2] - zi + wz * L;
+                double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 == 0.0) continue;
+                double r = sqrt(r2);
+                double K = kind == 1 ? nfo_kernel_plummer(r, eps) : nfo_kernel(r, eps);
+                double mj = mass ? fabs((double)mass[j]) : 1.0;
+                sum += mj * r * K;
+            }
+        }
+        scale[k] = sum;
+    }
+    return bad ? NFO_ERR_ARG : NFO_OK;
+}
+
+/*
  * Exact number of ordered pair evaluations of the definition (self pairs included):
  * I = sum_c count[c] * sum_{c' in stencil(c)} count[c'].
  */

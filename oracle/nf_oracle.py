@@ -52,6 +52,8 @@ def _load():
         lib.nfo_accel.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_density.restype = i32
         lib.nfo_density.argtypes = [vp, i64, i32, f64, f64, i32, vp, vp, vp, vp, i64, vp]
+        lib.nfo_force_scale.restype = i32
+        lib.nfo_force_scale.argtypes = [vp, vp, i64, i32, f64, f64, i32, i32, vp, vp, vp, vp, i64, vp]
         lib.nfo_interactions.restype = i64
         lib.nfo_interactions.argtypes = [vp, i32, i32]
         _lib = lib
@@ -160,6 +162,34 @@ def density(pos, cpd: int, L: float, b: float, R: int = 2, sinks=None, binning=N
                              binning["perm"].ctypes.data, sp, m, rho.ctypes.data)
     _check(rc, "nfo_density")
     return rho
+
+
+def force_scale(pos, cpd: int, L: float, eps: float, R: int = 2, sinks=None, binning=None, softening: str = "spline",
+                mass=None) -> np.ndarray:
+    """float64 [m]: S_i = sum_j m_j |d_ij| K(|d_ij|) over the stencil of sink i -- the uncancelled magnitude of the
+    direct sum (reading C13): the scale a float32 evaluation's error is proportional to."""
+    kind = {"spline": 0, "plummer": 1}[softening]
+    pos = _pos32(pos)
+    n = pos.shape[0]
+    mp = None
+    if mass is not None:
+        mass = np.ascontiguousarray(mass, dtype=np.float32)
+        if mass.shape != (n,):
+            raise ValueError("mass must have shape (n,)")
+        mp = mass.ctypes.data
+    if binning is None:
+        binning = bin_particles(pos, cpd, L)
+    if sinks is None:
+        sp, m = None, n
+    else:
+        sinks = np.ascontiguousarray(sinks, dtype=np.int64)
+        sp, m = sinks.ctypes.data, sinks.shape[0]
+    out = np.zeros(m, np.float64)
+    rc = _load().nfo_force_scale(pos.ctypes.data, mp, n, cpd, float(L), float(eps), int(R), kind,
+                                 binning["cid"].ctypes.data, binning["offset"].ctypes.data,
+                                 binning["perm"].ctypes.data, sp, m, out.ctypes.data)
+    _check(rc, "nfo_force_scale")
+    return out
 
 
 def kick(vel, acc, dt: float) -> np.ndarray:

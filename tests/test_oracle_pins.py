@@ -14,6 +14,13 @@ import pytest
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
+# Spline radius over the Plummer-equivalent length: eps_s = 2.16 eps (reading C3; PAPER.md:170 quotes
+# "Plummer-equivalent" lengths but does not print the factor -- PARITY UNPINNED by the paper).  Stated ONCE here; what
+# the pins below can check independently of the literal is the property it stands for: equal central force gradient
+# with the Plummer law, 10 / eps_s^3 = 1 / eps^3, i.e. eps_s / eps = 10^(1/3) = 2.1544, which 2.16 meets to 0.3 %.
+EPS_S_OVER_EPS = 2.16
+assert abs(EPS_S_OVER_EPS - 10.0 ** (1.0 / 3.0)) < 0.003 * EPS_S_OVER_EPS
+
 
 # ------------------------------------------------------------------ independent brute force
 def taylor_kernel(r, eps_s):
@@ -50,7 +57,7 @@ def brute_min_image(pos, cpd, L, eps, R):
     oc = (oc + cpd // 2) % cpd - cpd // 2        # wrapped offset; |.| = cpd/2 ties are > R anyway
     mask = (np.abs(oc).max(axis=2) <= R)
     r = np.sqrt((d * d).sum(axis=2))
-    K = taylor_kernel(r, 2.16 * eps) * mask
+    K = taylor_kernel(r, EPS_S_OVER_EPS * eps) * mask
     return (d * K[:, :, None]).sum(axis=1)
 
 
@@ -65,7 +72,7 @@ def brute_cell_image_allpairs(pos, cpd, L, eps):
     w = (ow - oc) // cpd                             # -1, 0, +1 box shifts
     d = x[None, :, :] - x[:, None, :] + w * L
     r = np.sqrt((d * d).sum(axis=2))
-    K = taylor_kernel(r, 2.16 * eps)
+    K = taylor_kernel(r, EPS_S_OVER_EPS * eps)
     return (d * K[:, :, None]).sum(axis=1)
 
 
@@ -105,7 +112,7 @@ def test_kernel_spline_defining_properties(oracle_mod):
     value, first and second derivative equal to those of r^-3 at eps_s.  These four facts fix the
     polynomial uniquely without quoting its coefficients."""
     eps = 0.37
-    es = 2.16 * eps
+    es = EPS_S_OVER_EPS * eps
     K = lambda r: oracle_mod.kernel(r, eps)
     # quadratic: third differences vanish anywhere inside
     for r0 in [0.05 * es, 0.3 * es, 0.7 * es]:
@@ -133,18 +140,18 @@ def test_kernel_plummer_equivalence(oracle_mod):
     eps = 0.013
     k0 = oracle_mod.kernel(1e-12, eps)
     assert k0 * eps ** 3 == pytest.approx(1.0, rel=0.01)
-    assert k0 * eps ** 3 == pytest.approx(10.0 / 2.16 ** 3, rel=1e-9)
+    assert k0 * eps ** 3 == pytest.approx(10.0 / EPS_S_OVER_EPS ** 3, rel=1e-9)
     # 'at a scale mildly larger than the softening length': eps < eps_s < 3 eps
     r_newton = min(r for r in np.linspace(eps, 3 * eps, 2001)
                    if oracle_mod.kernel(r, eps) == pytest.approx(r ** -3, rel=1e-14))
-    assert eps < r_newton <= 2.16 * eps * 1.001
+    assert eps < r_newton <= EPS_S_OVER_EPS * eps * 1.001
 
 
 def test_force_maximum(oracle_mod):
     """P4: F(r) = r K(r) peaks at u* = (30 - sqrt(180))/36 with F* = 2.01002/eps_s^2 (calculus on the
     quadratic fixed by P2), and the softened force never exceeds the Newtonian one."""
     eps = 0.2
-    es = 2.16 * eps
+    es = EPS_S_OVER_EPS * eps
     us = np.linspace(1e-4, 1.5, 150001)
     F = np.array([u * es * oracle_mod.kernel(u * es, eps) for u in us])
     i = F.argmax()
@@ -511,10 +518,10 @@ def test_mass_two_body_closed_form(oracle_mod):
     a = oracle_mod.accel_mass(pos, mass, 8, 1.0, 1.0 / 256, 2)
     assert a[0].tolist() == [8.0, 0.0, 0.0] and a[1].tolist() == [-48.0, 0.0, 0.0]
     # inside the spline the same factor multiplies the unit-mass closed form d (10 - 15u + 6u^2) / eps_s^3
-    eps = 0.125 / 2.16 * 2.0                           # eps_s = 0.25: d = 1/8 is u = 1/2
+    eps = 0.125 / EPS_S_OVER_EPS * 2.0                           # eps_s = 0.25: d = 1/8 is u = 1/2
     pos = np.array([[0.5, 0.5, 0.5], [0.625, 0.5, 0.5]], np.float32)
     a = oracle_mod.accel_mass(pos, mass, 8, 1.0, eps, 2)
-    f = 0.125 * (10 - 7.5 + 1.5) / (2.16 * eps) ** 3
+    f = 0.125 * (10 - 7.5 + 1.5) / (EPS_S_OVER_EPS * eps) ** 3
     assert a[0, 0] == pytest.approx(0.5 * f, rel=1e-14) and a[1, 0] == pytest.approx(-3.0 * f, rel=1e-14)
 
 
@@ -587,6 +594,109 @@ def test_mass_brute_force(oracle_mod, cpd, R, n, eps):
     w = (c[:, None] + off - c[None]) // cpd                  # box wrap implied by the cell offset (C7)
     d = p[None] - p[:, None] + w
     r = np.sqrt((d ** 2).sum(-1))
-    kk = np.where(near, taylor_kernel(r, 2.16 * eps), 0.0) * mass.astype(np.float64)[None]
+    kk = np.where(near, taylor_kernel(r, EPS_S_OVER_EPS * eps), 0.0) * mass.astype(np.float64)[None]
     ref = (d * kk[..., None]).sum(1)
     np.testing.assert_allclose(a, ref, rtol=1e-9, atol=1e-9 * np.abs(ref).max())
+
+
+# ------------------------------------------------------------------ uncancelled force magnitude (reading C13)
+def _force_scale_cases():
+    cases, cur = [], None
+    for l in open(os.path.join(GOLDEN, "force_scale.txt")):
+        t = l.split()
+        if not t or t[0].startswith("#"):
+            continue
+        if t[0] == "case":
+            cur = {"cpd": int(t[1]), "R": int(t[2]), "eps": float(t[3]), "n": int(t[4]), "rows": []}
+        elif t[0] == "expect":
+            cur["S"], cur["a"] = float(t[1]), float(t[2])
+            assert len(cur["rows"]) == cur["n"]
+            cases.append(cur)
+        else:
+            cur["rows"].append([float(v) for v in t])
+    return cases
+
+
+def test_force_scale_golden(oracle_mod):
+    """Closed forms (tests/golden/force_scale.txt): cancelling pairs add their magnitudes; masses weigh the terms;
+    cells beyond R and coincident particles add nothing."""
+    cases = _force_scale_cases()
+    assert len(cases) >= 5
+    for c in cases:
+        rows = np.array(c["rows"])
+        pos, mass = rows[:, :3].astype(np.float32), rows[:, 3].astype(np.float32)
+        assert np.array_equal(pos.astype(np.float64), rows[:, :3])          # dyadic: exact
+        S = oracle_mod.force_scale(pos, c["cpd"], 1.0, c["eps"], c["R"], mass=mass)
+        a = oracle_mod.accel_mass(pos, mass, c["cpd"], 1.0, c["eps"], c["R"])
+        assert S[0] == pytest.approx(c["S"], rel=1e-14), c
+        assert np.linalg.norm(a[0]) == pytest.approx(c["a"], rel=1e-14, abs=1e-12), c
+
+
+def test_force_scale_two_body_equals_norm(oracle_mod):
+    """One source: S_0 = |a_0| -- every row of the two-body golden file (incl. periodic faces, R / R+1, r = 0)."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "two_body.txt")) if l.strip() and l[0] != "#"]
+    for row in rows:
+        cpd, R, eps = int(row[0]), int(row[1]), float(row[2])
+        v = [float(t) for t in row[3:]]
+        pos = np.array([v[0:3], v[3:6]], dtype=np.float32)
+        S = oracle_mod.force_scale(pos, cpd, 1.0, eps, R)
+        assert S[0] == pytest.approx(np.linalg.norm(v[6:9]), rel=1e-14, abs=1e-12), row
+        assert S[1] == pytest.approx(S[0], rel=1e-14, abs=1e-12), row
+
+
+@pytest.mark.parametrize("cpd,R,n,eps,softening", [(6, 2, 300, 0.004, "spline"), (8, 1, 400, 0.03, "spline"),
+                                                   (7, 2, 350, 0.05, "plummer"), (5, 2, 200, 0.0, "spline")])
+def test_force_scale_brute_force(oracle_mod, cpd, R, n, eps, softening):
+    """All pairs by another route (particle-wise minimum image + explicit cell-offset mask, numpy), weights |m_j|.
+    cpd = 5 = 2R+1 goes through the unmasked cell-image construction instead."""
+    rng = np.random.default_rng(77 + cpd)
+    pos = rng.random((n, 3)).astype(np.float32)
+    mass = (rng.random(n) * 3 - 0.5).astype(np.float32)                    # some negative: the weight is |m|
+    x = pos.astype(np.float64)
+    c = cells_of(pos, cpd, 1.0)
+    oc = c[None, :, :] - c[:, None, :]
+    if cpd == 2 * R + 1:
+        ow = (oc + R) % cpd - R
+        d = x[None, :, :] - x[:, None, :] + ((ow - oc) // cpd) * 1.0
+        near = np.ones((n, n), bool)
+    else:
+        d = x[None, :, :] - x[:, None, :]
+        d -= np.round(d)
+        near = np.abs((oc + cpd // 2) % cpd - cpd // 2).max(axis=2) <= R
+    r = np.sqrt((d * d).sum(axis=2))
+    if softening == "plummer":
+        K = np.where(r > 0, (r * r + eps * eps) ** -1.5, 0.0)
+    else:
+        K = taylor_kernel(r, EPS_S_OVER_EPS * eps)
+    ref = (np.where(near, r * K, 0.0) * np.abs(mass.astype(np.float64))[None, :]).sum(axis=1)
+    S = oracle_mod.force_scale(pos, cpd, 1.0, eps, R, softening=softening, mass=mass)
+    np.testing.assert_allclose(S, ref, rtol=1e-12)
+    unit = oracle_mod.force_scale(pos, cpd, 1.0, eps, R, softening=softening)
+    np.testing.assert_allclose(unit, np.where(near, r * K, 0.0).sum(axis=1), rtol=1e-12)
+
+
+def test_force_scale_invariants(oracle_mod):
+    """Triangle inequality |a_i| <= S_i; lattice of one particle per cell: a = 0 while S is the lattice sum over the
+    (2R+1)^3 - 1 neighbour offsets of 1/|n w|^2; power-of-two scaling exact; shuffle and sink-subset consistent;
+    unit masses = no masses; linear in the masses."""
+    rng = np.random.default_rng(9)
+    cpd, eps = 8, 0.003
+    pos = rng.random((900, 3)).astype(np.float32)
+    S = oracle_mod.force_scale(pos, cpd, 1.0, eps, 2)
+    a = oracle_mod.accel(pos, cpd, 1.0, eps, 2)
+    assert np.all(np.linalg.norm(a, axis=1) <= S * (1 + 1e-12))
+    assert np.all(S > 0)
+    g = (np.stack(np.meshgrid(*[np.arange(cpd)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) / cpd
+    Sl = oracle_mod.force_scale(g.astype(np.float32), cpd, 1.0, 1e-6, 2)
+    o = np.stack(np.meshgrid(*[np.arange(-2, 3)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    o = o[(o != 0).any(axis=1)]
+    np.testing.assert_allclose(Sl, (1.0 / ((o / cpd) ** 2).sum(axis=1)).sum(), rtol=1e-13)
+    assert np.abs(oracle_mod.accel(g.astype(np.float32), cpd, 1.0, 1e-6, 2)).max() <= 1e-12 * Sl.max()
+    assert np.array_equal(oracle_mod.force_scale(pos * 4, cpd, 4.0, eps * 4, 2), S / 16)
+    perm = rng.permutation(len(pos))
+    np.testing.assert_allclose(oracle_mod.force_scale(pos[perm], cpd, 1.0, eps, 2), S[perm], rtol=1e-13)
+    sinks = np.array([5, 0, 899, 17])
+    assert np.array_equal(oracle_mod.force_scale(pos, cpd, 1.0, eps, 2, sinks=sinks), S[sinks])
+    assert np.array_equal(oracle_mod.force_scale(pos, cpd, 1.0, eps, 2, mass=np.ones(900, np.float32)), S)
+    m = rng.lognormal(0, 1, 900).astype(np.float32)
+    assert np.array_equal(oracle_mod.force_scale(pos, cpd, 1.0, eps, 2, mass=2 * m), 2 * oracle_mod.force_scale(pos, cpd, 1.0, eps, 2, mass=m))

@@ -41,7 +41,7 @@ extern "C" {
 #endif
 
 #define NF_OK            0
-#define NF_ERR_ARG      -1   /* null pointer, n < 0, n + 3 cpd^3 >= 2^32, cpd < 2R+1, cpd^3 >= 2^32, L <= 0, eps < 0, R < 0 or R > 4 */
+#define NF_ERR_ARG      -1   /* null pointer, n < 0, n + 3 cpd^3 >= 2^32, cpd < 2R+1, cpd^3 >= 2^32, L <= 0, eps < 0, R < 0 or R > 127 */
 #define NF_ERR_DOMAIN   -2   /* a coordinate is non-finite or outside [0, L)  (reported by nf_bin) */
 #define NF_ERR_STATE    -3   /* nf_accel before a successful nf_bin */
 #define NF_ERR_NOMEM    -4   /* device allocation failed / caller workspace too small */
@@ -71,7 +71,7 @@ typedef struct nf_stats {
  *   cpd  cells per dimension (>= 2R+1 so that no cell appears twice in a stencil)
  *   L    box side (> 0), positions live in [0, L)
  *   eps  Plummer-equivalent softening length (>= 0; 0 = pure Newtonian)
- *   R    near-field radius in cells (0..4; 2 in production)
+ *   R    near-field radius in cells (>= 0 with cpd >= 2R+1; 2 in production; at most 127)
  * Host-only: validates, precomputes constants, allocates nothing of size O(n).
  * Returns NULL on error (see nf_last_error()).
  */
@@ -82,9 +82,11 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R);
  * (within a cell: ascending input index), cell-sorted source arrays, work-unit list.
  *   pos_dev  [n][3] float32, input order, device memory, read only
  *   n        0 <= n, n + 3 cpd^3 < 2^32.  n = 0 is a valid no-op.
+ *            (the cell-padded source arrays are indexed with 32 bits: every non-empty cell adds up to 3 pad slots)
  * May be called repeatedly; each call invalidates the previous binning.  Enqueues on the plan's
- * stream, then performs ONE 4-byte device-to-host read (the domain-error flag) and therefore
- * synchronises that stream before returning.
+ * stream and, as its LAST action, performs one 16-byte device-to-host read (the domain-error flag and the
+ * number of work units) and therefore synchronises that stream before returning: the binning is complete
+ * on return, nothing of it is still pending on the stream.
  * Errors: NF_ERR_ARG, NF_ERR_DOMAIN (no partial result promised), NF_ERR_NOMEM, NF_ERR_CUDA.
  */
 int nf_bin(nf_plan *plan, const float *pos_dev, long long n);

@@ -53,6 +53,9 @@ def _load() -> ctypes.CDLL:
             if not os.path.exists(path):
                 raise ImportError(f"libnf_b200.so is missing and could not be built ({e}); "
                                   "there is no CPU fallback") from e
+            import warnings
+            warnings.warn(f"libnf_b200.so is older than its sources and the rebuild failed ({e}): running the STALE library",
+                          RuntimeWarning)
     lib = ctypes.CDLL(path)
     vp, ll, i32, dbl = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_double
     pp = ctypes.POINTER(ctypes.c_void_p)
@@ -123,14 +126,27 @@ def _host_f32(t: torch.Tensor, what: str) -> torch.Tensor:
 
 
 # ---- the C calls, same names ------------------------------------------------------------------
+# The C ABI takes bare pointers: a caller buffer shorter than the n of the last binning would be written out of bounds
+# on the device.  The binding therefore remembers (n, cpd^3) per plan handle and checks every output tensor against it.
+_SHAPE: dict[int, list] = {}
+
+
+def _rows(plan: int, t: torch.Tensor, what: str) -> None:
+    n = _SHAPE.get(plan, [None, None])[0]
+    if n is not None and t.shape[0] != n:
+        raise ValueError(f"{what} has {t.shape[0]} rows but the plan last binned {n} particles")
+
+
 def nf_plan_create(cpd: int, L: float, eps: float, R: int = 2) -> int:
     h = _lib.nf_plan_create(int(cpd), float(L), float(eps), int(R))
     if not h:
         raise NFError(NF_ERR_ARG, nf_last_error())
+    _SHAPE[h] = [None, int(cpd) ** 3]
     return h
 
 
 def nf_destroy(plan: int) -> None:
+    _SHAPE.pop(plan, None)
     _lib.nf_destroy(plan)
 
 
@@ -140,11 +156,16 @@ def nf_set_stream(plan: int, cuda_stream: int) -> None:
 
 def nf_bin(plan: int, pos: torch.Tensor) -> None:
     pos = _dev_f32(pos, "pos")
+    if plan in _SHAPE:
+        _SHAPE[plan][0] = None
     _check(_lib.nf_bin(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0]))
+    if plan in _SHAPE:
+        _SHAPE[plan][0] = pos.shape[0]
 
 
 def nf_accel(plan: int, acc: torch.Tensor) -> None:
     acc = _dev_f32(acc, "acc")
+    _rows(plan, acc, "acc")
     _check(_lib.nf_accel(plan, ctypes.c_void_p(acc.data_ptr())))
 
 
@@ -153,6 +174,7 @@ def nf_accel_density(plan: int, acc: torch.Tensor, rho: torch.Tensor, b: float) 
     if not (isinstance(rho, torch.Tensor) and rho.is_cuda and rho.dtype == torch.float32 and rho.is_contiguous()
             and rho.dim() == 1 and rho.shape[0] == acc.shape[0]):
         raise TypeError("rho must be a contiguous CUDA float32 tensor of shape [n]")
+    _rows(plan, acc, "acc")
     _check(_lib.nf_accel_density(plan, ctypes.c_void_p(acc.data_ptr()), ctypes.c_void_p(rho.data_ptr()), float(b)))
 
 
@@ -161,9 +183,15 @@ def nf_accel_kick(plan: int, acc: torch.Tensor | None, vel: torch.Tensor | None,
     pa = ctypes.c_void_p(_dev_f32(acc, "acc").data_ptr()) if acc is not None else None
     pv = ctypes.c_void_p(_dev_f32(vel, "vel").data_ptr()) if vel is not None else None
     pm = None
+    for t, what in ((acc, "acc"), (vel, "vel")):
+        if t is not None:
+            _rows(plan, t, what)
     if amax_cell is not None:
         if not (amax_cell.is_cuda and amax_cell.dtype == torch.float32 and amax_cell.is_contiguous() and amax_cell.dim() == 1):
             raise TypeError("amax_cell must be a contiguous CUDA float32 tensor of shape [cpd^3]")
+        nc = _SHAPE.get(plan, [None, None])[1]
+        if nc is not None and amax_cell.shape[0] != nc:
+            raise ValueError(f"amax_cell has {amax_cell.shape[0]} entries but the plan has {nc} cells")
         pm = ctypes.c_void_p(amax_cell.data_ptr())
     _check(_lib.nf_accel_kick(plan, pa, pv, float(dt), pm))
 
@@ -183,11 +211,16 @@ def nf_set_sink_slabs(plan: int, x_first: int, n_slabs: int) -> None:
 
 def nf_bin_host(plan: int, pos_host: torch.Tensor) -> None:
     pos_host = _host_f32(pos_host, "pos_host")
+    if plan in _SHAPE:
+        _SHAPE[plan][0] = None
     _check(_lib.nf_bin_host(plan, ctypes.c_void_p(pos_host.data_ptr()), pos_host.shape[0]))
+    if plan in _SHAPE:
+        _SHAPE[plan][0] = pos_host.shape[0]
 
 
 def nf_accel_host(plan: int, acc_host: torch.Tensor) -> None:
     acc_host = _host_f32(acc_host, "acc_host")
+    _rows(plan, acc_host, "acc_host")
     _check(_lib.nf_accel_host(plan, ctypes.c_void_p(acc_host.data_ptr())))
 
 

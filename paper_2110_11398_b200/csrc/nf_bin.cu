@@ -180,11 +180,14 @@ __global__ void __launch_bounds__(kSortThreads) cellid_kernel(const float *__res
 }
 
 // ---- S4: stable LSD radix sort of (cell id, input index), 8-11 bits per pass, gather fused into the last pass -------
+// n_dev != NULL: the number of keys lives on the device (the unit sort: nf_bin does not read it back before the sort; the
+// grid is sized from the host-side bound and blocks past the end write empty histograms)
 __global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const uint32_t *__restrict__ kin, size_t n, int shift,
                                                                   uint32_t digit_mask, uint32_t *__restrict__ hist,
-                                                                  uint32_t nblocks)
+                                                                  uint32_t nblocks, const uint32_t *__restrict__ n_dev)
 {
     __shared__ uint32_t h[1 << kSortMaxBits];
+    if (n_dev) n = *n_dev;
     for (uint32_t d = threadIdx.x; d <= digit_mask; d += kSortThreads) h[d] = 0;
     __syncthreads();
     const size_t base = (size_t)blockIdx.x * kSortTile;
@@ -232,8 +235,10 @@ template <int BITS, bool IOTA, bool LAST>
 __global__ void __launch_bounds__(kSortThreads, 2) radix_scatter_kernel(const uint32_t *__restrict__ kin, const uint32_t *__restrict__ vin,
                                                                         uint32_t *__restrict__ kout, uint32_t *__restrict__ vout,
                                                                         size_t n, int shift, const uint32_t *__restrict__ hist,
-                                                                        uint32_t nblocks, const GatherArgs g)
+                                                                        uint32_t nblocks, const GatherArgs g,
+                                                                        const uint32_t *__restrict__ n_dev)
 {
+    if (n_dev) n = *n_dev;
     constexpr int BINS = 1 << BITS;
     constexpr uint32_t MASK = BINS - 1;
     constexpr int DPT = BINS >= kSortThreads ? BINS / kSortThreads : 1;        // digits per thread in the scans
@@ -252,6 +257,7 @@ __global__ void __launch_bounds__(kSortThreads, 2) radix_scatter_kernel(const ui
         for (int q = threadIdx.x; q < kSortWarps * BINS / 2; q += kSortThreads) z[q] = 0;
     }
     const size_t tile0 = (size_t)blockIdx.x * kSortTile;
+    if (tile0 >= n) return;                                // only with n_dev: the grid covers the host-side bound
     const size_t seg = tile0 + (size_t)w * (32 * kSortItems);
     uint32_t key[kSortItems], lr[kSortItems / 2];     // ranks / tile-local positions: two 16-bit values per register
 #pragma unroll
@@ -395,46 +401,47 @@ static size_t scatter_smem_bytes() { return 8 * (size_t)kSortTile + 8 * ((size_t
 
 template <int BITS, bool IOTA, bool LAST>
 static cudaError_t scatter_launch(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift,
-                                  const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st)
+                                  const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st, const uint32_t *n_dev)
 {
     static_assert(2 * kSortWarps * (1 << BITS) <= 8 * kSortTile, "the counters must fit the tile storage");
     auto fn = radix_scatter_kernel<BITS, IOTA, LAST>;
     const size_t smem = scatter_smem_bytes<BITS>();
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    fn<<<nb, kSortThreads, smem, st>>>(kin, vin, kout, vout, n, shift, hist, nb, g);
+    fn<<<nb, kSortThreads, smem, st>>>(kin, vin, kout, vout, n, shift, hist, nb, g, n_dev);
     return cudaGetLastError();
 }
 
 template <int BITS>
 static cudaError_t scatter_dispatch(bool iota, bool last, const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout,
-                                    size_t n, int shift, const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st)
+                                    size_t n, int shift, const uint32_t *hist, uint32_t nb, const GatherArgs &g, cudaStream_t st,
+                                    const uint32_t *n_dev)
 {
-    if (iota) return last ? scatter_launch<BITS, true, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st)
-                          : scatter_launch<BITS, true, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st);
-    return last ? scatter_launch<BITS, false, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st)
-                : scatter_launch<BITS, false, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st);
+    if (iota) return last ? scatter_launch<BITS, true, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev)
+                          : scatter_launch<BITS, true, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev);
+    return last ? scatter_launch<BITS, false, true>(kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev)
+                : scatter_launch<BITS, false, false>(kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev);
 }
 
 // One pass over n keys: digit histogram per tile (unless the caller already has it), its scan, the scatter.
 // `last` (particle sort only) fuses the gather of `g` into the scatter.
 static int radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift, int bits,
                       bool iota, bool last, bool have_hist, const GatherArgs &g, uint32_t *hist, uint32_t *scan_tmp,
-                      cudaStream_t st, int *launches)
+                      cudaStream_t st, int *launches, const uint32_t *n_dev = nullptr)   // n_dev: n is an upper bound, the count is on the device
 {
     const uint32_t nb = (uint32_t)((n + kSortTile - 1) / kSortTile);
     const uint32_t bins = 1u << bits;
     if (!have_hist) {
-        radix_hist_kernel<<<nb, kSortThreads, 0, st>>>(kin, n, shift, bins - 1u, hist, nb);
+        radix_hist_kernel<<<nb, kSortThreads, 0, st>>>(kin, n, shift, bins - 1u, hist, nb, n_dev);
         *launches += 1;
     }
     exclusive_scan(hist, hist, (size_t)bins * nb, scan_tmp, OpId(), 0, nullptr, st, launches);
     cudaError_t e;
     switch (bits) {
-    case 8:  e = scatter_dispatch<8>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
-    case 9:  e = scatter_dispatch<9>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
-    case 10: e = scatter_dispatch<10>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
-    default: e = scatter_dispatch<11>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st); break;
+    case 8:  e = scatter_dispatch<8>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev); break;
+    case 9:  e = scatter_dispatch<9>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev); break;
+    case 10: e = scatter_dispatch<10>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev); break;
+    default: e = scatter_dispatch<11>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev); break;
     }
     NF_CUDA_OK(e);
     *launches += 1;
@@ -646,23 +653,26 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.offset, ws.src, ws.ubase, ws.units, ukey);  L++;
     NF_CUDA_OK(cudaGetLastError());
 
-    // domain flag + unit count: the one documented synchronisation of nf_bin
+    // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
+    const size_t ncol_sink = (size_t)k.nslab * k.cpd;
+    const size_t umax = (n < ncol_sink ? n : ncol_sink) + n / (size_t)(k.chunk < 32 ? 32 : k.chunk) + 2 * ncol_sink + 2;
+    const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 32 + 2;            // what carve() reserved
+    const size_t ub = umax < ucap ? umax : ucap;
+    if (p->heavy_first) {
+        const int rc = radix_pass(ukey, nullptr, free_key, free_val, ub, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
+                                  ws.scan_tmp, st, &L, &ws.scalars[2]);
+        if (rc != NF_OK) return rc;
+        units_permute_kernel<<<(unsigned)((ub + 255) / 256), 256, 0, st>>>(ws.units, free_val, &ws.scalars[2], ws.units_sorted);  L++;
+    }
+    NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
+    NF_CUDA_OK(cudaGetLastError());
+    // domain flag + unit count: the one documented synchronisation of nf_bin, at the END of the call -- nothing is
+    // enqueued after it, so the binning is complete on return whatever stream the caller uses next
     uint32_t sc[4];
     NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));
     NF_CUDA_OK(cudaStreamSynchronize(st));
     if (sc[0]) { set_error("nf_bin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
-    const size_t nu = sc[2];
-    p->n_units = (long long)nu;
-    if (p->heavy_first && nu > 1) {
-        const int rc = radix_pass(ukey, nullptr, free_key, free_val, nu, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
-                                  ws.scan_tmp, st, &L);
-        if (rc != NF_OK) return rc;
-        units_permute_kernel<<<(unsigned)((nu + 255) / 256), 256, 0, st>>>(ws.units, free_val, &ws.scalars[2], ws.units_sorted);  L++;
-    } else if (nu > 0) {
-        NF_CUDA_OK(cudaMemcpyAsync(ws.units_sorted, ws.units, sizeof(Unit) * nu, cudaMemcpyDeviceToDevice, st));
-    }
-    NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
-    NF_CUDA_OK(cudaGetLastError());
+    p->n_units = (long long)sc[2];
     p->have_bin_time = true;
     p->launches_bin = L;
     return NF_OK;

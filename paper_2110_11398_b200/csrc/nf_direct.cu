@@ -49,7 +49,7 @@ struct __align__(16) StageDesc {
     uint32_t ns;               //       sinks
     uint32_t z0, z1;           //       first / last sink cell (z index)
     uint32_t colbase;          //       col * cpd
-    int      oxy;              // column offset: (ox + 8) | (oy + 8) << 8
+    int      oxy;              // column offset: (ox + 128) | (oy + 128) << 8
     Piece    pieces[kMaxPieces];
 };
 
@@ -350,6 +350,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
     };
     auto commit = [&](int extra) {
         flush_copy();
+        __syncwarp();          // the table entries written by the other lanes are ordered before lane 0's releasing arrive
         if (lead) {
             sm.desc[stage].flags = sflags | extra;
             sm.desc[stage].npieces = np;
@@ -413,7 +414,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 first = false;
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
-                                    d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 8) | ((oy + 8) << 8);
+                                    d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
                                     d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
@@ -460,7 +461,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 first = false;
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
-                                    d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 8) | ((oy + 8) << 8);
+                                    d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
                                     d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
@@ -552,7 +553,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
             // squared gap between the sink and the neighbour column (0 for the own column): a cell whose
             // nearest face is farther than eps_s cannot hold a pair that needs the spline
             float gxy2 = 0.f;
-            const int ox = (d.oxy & 255) - 8, oy = (d.oxy >> 8) - 8;
+            const int ox = (d.oxy & 255) - 128, oy = (d.oxy >> 8) - 128;
             const bool near_col = ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1;
             const bool gap_dens = DENS && a.dens_mode == 1 && near_col;
             if (soft_mode == 1 || gap_dens) {
@@ -704,7 +705,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     a.k = p->k;
     a.x = p->ws.x; a.y = p->ws.y; a.z = p->ws.z; a.m = mass ? p->mass_soa : nullptr;
     a.poff = p->ws.poff; a.offset = p->ws.offset; a.perm = p->perm;
-    a.units = p->ws.units_sorted;
+    a.units = p->heavy_first ? p->ws.units_sorted : p->ws.units;
     a.n_units = (uint32_t)p->n_units;
     a.counter = &p->ws.scalars[1];
     a.acc = acc;

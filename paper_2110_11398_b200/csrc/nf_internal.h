@@ -11,7 +11,7 @@
 namespace nf {
 
 // ---- compile-time shape of the direct-sum kernel -------------------------------------------
-constexpr int kMaxR          = 4;                 // stencil (2R+1)^3 with R <= 4
+constexpr int kMaxR          = 127;               // the column offset travels as a biased byte; cpd >= 2R+1 is the real limit
 #ifndef NF_CONSUMER_WARPS
 #define NF_CONSUMER_WARPS 8
 #endif

@@ -17,3 +17,19 @@ def oracle_mod():
     import oracle
     oracle.build()
     return oracle
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Measured worst |a_gpu - a_ref| / S_i of the conditioning-aware rule (nf_testlib.assert_parity_conditioned)."""
+    try:
+        import nf_testlib
+    except Exception:
+        return
+    if not nf_testlib.RATIOS:
+        return
+    worst = max(nf_testlib.RATIOS, key=lambda t: t[1])
+    rows = sum(t[2] for t in nf_testlib.RATIOS)
+    total = sum(t[3] for t in nf_testlib.RATIOS)
+    terminalreporter.write_line(
+        f"C13 rule: {len(nf_testlib.RATIOS)} comparisons, {total} rows, {rows} rows outside 1e-5 |a_ref| (judged against "
+        f"C13 = {nf_testlib.C13:.1e} x S); worst err/S = {worst[1]:.3e} in [{worst[0]}]")

@@ -73,12 +73,34 @@ def sampled_check(oracle_mod, cfg, device="cpu"):
     print(cfg.name, "sampled sinks", len(sinks), st, out["stats"])
 
 
-def test_config2_full_size_sampled(oracle_mod):
-    sampled_check(oracle_mod, nf_inputs.config(2))
+def full_size_full_oracle(oracle_mod, cfg):
+    """EVERY particle of a full-size config against the oracle (full oracle on configs 1-3).  The maximum
+    of BASELINE.json's rule is set by the most-cancelled particle of the whole set, which a sink sample does not bound."""
+    pos_cpu = nf_inputs.generate(cfg)
+    out = gpu_run(pos_cpu, cfg.cpd, cfg.L, cfg.eps, cfg.R, want_binning=True)
+    pos = pos_cpu.numpy()
+    b = oracle_mod.bin_particles(pos, cfg.cpd, cfg.L)
+    assert_binning_equal(out["binning"], b)
+    assert out["stats"]["interactions"] == oracle_mod.interactions(b["count"], cfg.cpd, cfg.R)
+    ref = oracle_mod.accel(pos, cfg.cpd, cfg.L, cfg.eps, cfg.R, binning=b)
+    st = assert_parity(out["acc"], ref, cfg.name + " (all particles)")
+    a = out["acc"]
+    assert np.abs(a.sum(axis=0)).max() <= 2e-6 * np.abs(a).sum()
+    print(cfg.name, "ALL", len(ref), "particles", st, out["stats"])
+
+
+def test_config2_full_size_full_oracle(oracle_mod):
+    """1.85e10 pair interactions in float64: about 35 s of the box's 16 host cores."""
+    full_size_full_oracle(oracle_mod, nf_inputs.config(2))
 
 
 def test_config3_full_size_sampled(oracle_mod):
     sampled_check(oracle_mod, nf_inputs.config(3))
+
+
+@pytest.mark.skipif(os.environ.get("NF_FULL_ORACLE") != "1", reason="1.41e11 float64 pair interactions (~4.5 min of 16 cores): NF_FULL_ORACLE=1; the result of the round-2 run is in DESIGN.md 5")
+def test_config3_full_size_full_oracle(oracle_mod):
+    full_size_full_oracle(oracle_mod, nf_inputs.config(3))
 
 
 def test_config4_full_size_sampled(oracle_mod):
@@ -89,10 +111,18 @@ def test_config5_full_size_sampled(oracle_mod):
     """Production-size config (1024^3 particles, ~26 GB of positions + accelerations): binning bit-exact at
     full N, accelerations on the sink sample.  Needs ~60 GB of host memory for the oracle's arrays."""
     import psutil
+    need = []
     if psutil.virtual_memory().available < 70 * 2 ** 30:
-        pytest.skip("needs 70 GB of free host memory")
+        need.append("70 GB of free host memory")
     if torch.cuda.mem_get_info()[0] < 120 * 2 ** 30:
-        pytest.skip("needs 120 GB of free device memory")
+        need.append("120 GB of free device memory")
+    if need:
+        # on the B200 box the production-size config must run: NF_REQUIRE_CONFIG5=1 turns the skip into a failure
+        # (set by the round's GPU runs, see DESIGN.md 5); elsewhere a smaller box skips visibly
+        msg = "config 5 needs " + " and ".join(need)
+        if os.environ.get("NF_REQUIRE_CONFIG5") == "1":
+            pytest.fail(msg + " (NF_REQUIRE_CONFIG5=1)")
+        pytest.skip(msg)
     cfg = nf_inputs.config(5)
     import paper_2110_11398_b200 as nf
     pos_dev = nf_inputs.generate(cfg, device="cuda")
@@ -195,10 +225,11 @@ def test_coincident_particles(oracle_mod):
 
 
 @pytest.mark.parametrize("cpd,R,eps,L", [(5, 2, 0.01, 1.0), (3, 1, 0.02, 1.0), (1, 0, 0.01, 1.0), (7, 3, 0.005, 1.0),
-                                         (9, 4, 0.004, 1.0), (6, 0, 0.01, 1.0), (6, 2, 0.2, 1.0), (6, 2, 0.0, 1.0),
+                                         (9, 4, 0.004, 1.0), (11, 5, 0.003, 1.0), (17, 8, 0.002, 1.0), (14, 6, 0.01, 3.0),
+                                         (6, 0, 0.01, 1.0), (6, 2, 0.2, 1.0), (6, 2, 0.0, 1.0),
                                          (8, 2, 0.03, 7.5), (8, 2, 25.0, 2000.0), (16, 2, 1e-5, 2.0 ** -10)])
 def test_parameter_sweep(oracle_mod, cpd, R, eps, L):
-    """cpd = 2R+1 (every cell in every stencil), R = 0..4, eps = 0, eps_s larger than a cell (no fast
+    """cpd = 2R+1 (every cell in every stencil), R = 0..8 (any R >= 0 with cpd >= 2R+1), eps = 0, eps_s larger than a cell (no fast
     path), non-unit and non-dyadic box sizes."""
     g = torch.Generator().manual_seed(cpd * 10 + R)
     pos = (torch.rand((4000, 3), generator=g, dtype=torch.float64) * L).to(torch.float32)
@@ -332,6 +363,18 @@ def test_errors_gpu():
                 p.accel(torch.empty((2, 3), device="cuda"))
         p.bin(torch.rand((10, 3), device="cuda"))      # the plan recovers
         p.accel()
+        # the binding refuses output buffers that do not match the last binning (the C ABI would write out of bounds)
+        with pytest.raises(ValueError):
+            p.accel(torch.empty((9, 3), device="cuda"))
+        with pytest.raises(ValueError):
+            nf.nf_accel_kick(p._h, None, None, 0.1, torch.empty(5, device="cuda"))
+        with pytest.raises(ValueError):
+            nf.nf_accel_kick(p._h, None, torch.zeros((11, 3), device="cuda"), 0.1, None)
+    # cpd < 2R+1 is the argument error, not R itself
+    with pytest.raises(nf.NFError) as e:
+        nf.Plan(10, 1.0, 0.01, 5)
+    assert e.value.code == B.NF_ERR_ARG
+    nf.Plan(11, 1.0, 0.01, 5).close()
 
 
 # ---------------------------------------------------------------- fused kernel density estimate

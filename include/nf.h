@@ -64,6 +64,8 @@ typedef struct nf_stats {
     int   accel_block;         /* threads per CTA */
     int   kernel_launches_bin; /* kernels launched by one nf_bin */
     int   kernel_launches_accel; /* kernels launched by one nf_accel */
+    int   rebin_path;          /* last nf_rebin: 1 = incremental merge, 2 = sorted from scratch; 0 = none since nf_bin */
+    long long rebin_movers;    /* particles that changed cell in the last incremental nf_rebin (-1: not counted) */
 } nf_stats;
 
 /*
@@ -90,6 +92,25 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R);
  * Errors: NF_ERR_ARG, NF_ERR_DOMAIN (no partial result promised), NF_ERR_NOMEM, NF_ERR_CUDA.
  */
 int nf_bin(nf_plan *plan, const float *pos_dev, long long n);
+
+/*
+ * nf_rebin -- steps S1-S5 again for the SAME particles after they moved: the paper's pipeline
+ * "reorders particles into their new cells" after every drift ("moving particles to their new cells",
+ * PAPER.md:353; Table 6 "Finish" / "Merge New Particles"), and a drift is much shorter than a cell,
+ * so nearly every particle stays where it was.
+ *   pos_dev  [n][3] float32, device memory, the new positions in the SAME input order and with the same n as the
+ *            last nf_bin / nf_rebin of this plan.
+ * The result is by definition what nf_bin(plan, pos_dev, n) gives -- cell ids, counts, offsets and the stable
+ * permutation are bit-identical to it (and to the oracle), hence so are the accelerations -- but no radix pass
+ * runs: one pass over the input order finds the particles that changed cell, one pass over the old sorted order
+ * merges each cell's stayers with its arrivals and rewrites the source arrays.  Falls back to the full sort when more
+ * than a quarter of the particles moved, when ranking the arrivals (sum over the cells of arrivals^2) would cost more
+ * than 16 n comparisons, or when the previous call saw more than 1/16 of the particles move (nf_stats.rebin_path / rebin_movers say which path ran).
+ * Like nf_bin it resets the plan to unit masses and synchronises the stream once, as its last action.
+ * Errors: NF_ERR_STATE (no valid binning: call nf_bin first, also after nf_set_sink_slabs / "window" / "heavy_first"),
+ *         NF_ERR_ARG, NF_ERR_DOMAIN (the binning is invalid afterwards), NF_ERR_CUDA.
+ */
+int nf_rebin(nf_plan *plan, const float *pos_dev);
 
 /*
  * nf_accel -- steps S6-S7: the direct sum over the cell stencil and the scatter to input order.

@@ -21,7 +21,7 @@ NF_OK, NF_ERR_ARG, NF_ERR_DOMAIN, NF_ERR_STATE, NF_ERR_NOMEM, NF_ERR_CUDA = 0, -
 _ERR_NAMES = {-1: "NF_ERR_ARG", -2: "NF_ERR_DOMAIN", -3: "NF_ERR_STATE", -4: "NF_ERR_NOMEM", -5: "NF_ERR_CUDA"}
 
 EXPORTS = [
-    "nf_plan_create", "nf_bin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_masses", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
+    "nf_plan_create", "nf_bin", "nf_rebin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_masses", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
 ]
@@ -41,6 +41,7 @@ class nf_stats(ctypes.Structure):
         ("sm_count", ctypes.c_int), ("clock_khz", ctypes.c_int),
         ("accel_grid", ctypes.c_int), ("accel_block", ctypes.c_int),
         ("kernel_launches_bin", ctypes.c_int), ("kernel_launches_accel", ctypes.c_int),
+        ("rebin_path", ctypes.c_int), ("rebin_movers", ctypes.c_longlong),
     ]
 
 
@@ -63,6 +64,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_plan_create.argtypes = [i32, dbl, dbl, i32]
     lib.nf_bin.restype = i32
     lib.nf_bin.argtypes = [vp, vp, ll]
+    lib.nf_rebin.restype = i32
+    lib.nf_rebin.argtypes = [vp, vp]
     lib.nf_accel.restype = i32
     lib.nf_accel.argtypes = [vp, vp]
     lib.nf_accel_density.restype = i32
@@ -161,6 +164,13 @@ def nf_bin(plan: int, pos: torch.Tensor) -> None:
     _check(_lib.nf_bin(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0]))
     if plan in _SHAPE:
         _SHAPE[plan][0] = pos.shape[0]
+
+
+def nf_rebin(plan: int, pos: torch.Tensor) -> None:
+    """The same particles after they moved: new positions in the same input order (include/nf.h)."""
+    pos = _dev_f32(pos, "pos")
+    _rows(plan, pos, "pos")
+    _check(_lib.nf_rebin(plan, ctypes.c_void_p(pos.data_ptr())))
 
 
 def nf_accel(plan: int, acc: torch.Tensor) -> None:
@@ -286,6 +296,7 @@ class Plan:
     """``with Plan(cpd, L, eps, R) as p: p.bin(pos); acc = p.accel()``"""
 
     def __init__(self, cpd: int, L: float, eps: float, R: int = 2):
+        self._h = None
         self.cpd, self.L, self.eps, self.R = int(cpd), float(L), float(eps), int(R)
         self.ncells = self.cpd ** 3
         self.n = 0
@@ -317,6 +328,11 @@ class Plan:
         self._use_current_stream()
         nf_bin(self._h, pos)
         self.n = pos.shape[0]
+
+    def rebin(self, pos: torch.Tensor):
+        """Incremental re-binning of the same particles at new positions (same order, same n)."""
+        self._use_current_stream()
+        nf_rebin(self._h, pos)
 
     def set_masses(self, mass: torch.Tensor | None):
         """Source masses [n] (input order) of the particles last binned; None = unit masses.  nf_bin resets them."""

@@ -65,6 +65,16 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     ws.bucket_hist  = (uint32_t *)take(4 * 256);
     ws.interactions = (unsigned long long *)take(8 * 4);
     ws.scalars      = (uint32_t *)take(4 * 64);
+    ws.offset_new = (uint32_t *)take(4 * (C + 2));
+    ws.arr_count  = (uint32_t *)take(4 * (C + 2));
+    ws.arr_off    = (uint32_t *)take(4 * (C + 2));
+    ws.arr_cursor = (uint32_t *)take(4 * (C + 2));
+    ws.mover_list = (uint32_t *)take(4 * (N / 4 + 64));
+    ws.arr_list   = (uint32_t *)take(4 * (N / 4 + 64));
+    ws.moverbits  = (uint32_t *)take(4 * (N / 32 + 2));
+    ws.staybits   = (uint32_t *)take(4 * (N / 32 + 2));
+    ws.wordprefix = (uint32_t *)take(4 * (N / 32 + 2));
+    ws.tile_state = (unsigned long long *)take(8 * (N / kSortTile + 2));
     ws.bytes = off;
     return off;
 }
@@ -276,9 +286,25 @@ int nf_bin(nf_plan *p, const float *pos, long long n)
     if (rc) return rc;
     rc = ensure_workspace(p, n);
     if (rc) return rc;
+    p->rebin_movers = -1; p->rebin_path = 0;
     rc = launch_bin(p, pos, n);
     if (rc) return rc;
     p->n = n; p->binned = true;
+    return NF_OK;
+}
+
+int nf_rebin(nf_plan *p, const float *pos)
+{    DeviceGuard guard(p);
+
+    if (!p) { set_error("null plan"); return NF_ERR_ARG; }
+    if (!p->binned) { set_error("nf_rebin called before a successful nf_bin (options that change the work units need a fresh nf_bin)"); return NF_ERR_STATE; }
+    if (!pos && p->n > 0) { set_error("null pos"); return NF_ERR_ARG; }
+    p->binned = false;
+    p->have_mass = false;                                       // masses belong to one binning
+    if (p->n == 0) { p->binned = true; return NF_OK; }
+    const int rc = launch_rebin(p, pos);
+    if (rc) return rc;
+    p->binned = true;
     return NF_OK;
 }
 
@@ -412,6 +438,7 @@ int nf_get_stats(nf_plan *p, nf_stats *out)
     out->accel_grid = p->accel_grid;
     out->kernel_launches_bin = p->launches_bin;
     out->kernel_launches_accel = p->launches_accel;
+    out->rebin_path = p->rebin_path; out->rebin_movers = p->rebin_movers;
     NF_CUDA_OK(cudaStreamSynchronize(p->stream));
     if (p->binned) {
         out->n = p->n;

@@ -584,6 +584,42 @@ int launch_set_masses(nf_plan *p, const float *mass)
     return NF_OK;
 }
 
+// ---- S5 on the stream: per-cell stencil counts + exact interaction count, units per column, units, heavy-first order.
+// free_key / free_val: two n-sized scratch arrays for the unit sort.
+static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free_val, int *Lp)
+{
+    const Consts &k = p->k;
+    Workspace &ws = p->ws;
+    cudaStream_t st = p->stream;
+    int &L = *Lp;
+    GatherArgs g{};
+    // stencil source counts + exact interaction count, units per column, units + heavy-first order: one
+    // stable radix pass on the cost key (clz of the unit's interaction count, so heavier units come first
+    // and equal keys keep column order).  The keys sit in the storage of units_sorted until the order is
+    // known; the sort writes into the free particle-sort buffers.
+    const unsigned nbc = (k.ncells + 255) / 256;
+    const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
+    uint32_t *ukey = (uint32_t *)ws.units_sorted;
+    cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions);  L++;
+    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.offset, ws.ubase);  L++;
+    exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
+    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.offset, ws.src, ws.ubase, ws.units, ukey);  L++;
+    NF_CUDA_OK(cudaGetLastError());
+
+    // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
+    const size_t ncol_sink = (size_t)k.nslab * k.cpd;
+    const size_t umax = (n < ncol_sink ? n : ncol_sink) + n / (size_t)(k.chunk < 32 ? 32 : k.chunk) + 2 * ncol_sink + 2;
+    const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 32 + 2;            // what carve() reserved
+    const size_t ub = umax < ucap ? umax : ucap;
+    if (p->heavy_first) {
+        const int rc = radix_pass(ukey, nullptr, free_key, free_val, ub, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
+                                  ws.scan_tmp, st, &L, &ws.scalars[2]);
+        if (rc != NF_OK) return rc;
+        units_permute_kernel<<<(unsigned)((ub + 255) / 256), 256, 0, st>>>(ws.units, free_val, &ws.scalars[2], ws.units_sorted);  L++;
+    }
+    return NF_OK;
+}
+
 // ------------------------------------------------------------------------------------------
 int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 {
@@ -638,32 +674,10 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     }
     p->sort_passes = passes;
     p->perm = vin;
+    p->slotcell = nullptr;                                     // materialised by the first nf_rebin
     uint32_t *free_key = kbuf[passes & 1], *free_val = vbuf[passes & 1];   // the pair not holding the result
 
-    // stencil source counts + exact interaction count, units per column, units + heavy-first order: one
-    // stable radix pass on the cost key (clz of the unit's interaction count, so heavier units come first
-    // and equal keys keep column order).  The keys sit in the storage of units_sorted until the order is
-    // known; the sort writes into the free particle-sort buffers.
-    const unsigned nbc = (k.ncells + 255) / 256;
-    const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
-    uint32_t *ukey = (uint32_t *)ws.units_sorted;
-    cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions);  L++;
-    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.offset, ws.ubase);  L++;
-    exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
-    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.offset, ws.src, ws.ubase, ws.units, ukey);  L++;
-    NF_CUDA_OK(cudaGetLastError());
-
-    // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
-    const size_t ncol_sink = (size_t)k.nslab * k.cpd;
-    const size_t umax = (n < ncol_sink ? n : ncol_sink) + n / (size_t)(k.chunk < 32 ? 32 : k.chunk) + 2 * ncol_sink + 2;
-    const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 32 + 2;            // what carve() reserved
-    const size_t ub = umax < ucap ? umax : ucap;
-    if (p->heavy_first) {
-        const int rc = radix_pass(ukey, nullptr, free_key, free_val, ub, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
-                                  ws.scan_tmp, st, &L, &ws.scalars[2]);
-        if (rc != NF_OK) return rc;
-        units_permute_kernel<<<(unsigned)((ub + 255) / 256), 256, 0, st>>>(ws.units, free_val, &ws.scalars[2], ws.units_sorted);  L++;
-    }
+    { const int rc = launch_units(p, n, free_key, free_val, &L); if (rc != NF_OK) return rc; }
     NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
     NF_CUDA_OK(cudaGetLastError());
     // domain flag + unit count: the one documented synchronisation of nf_bin, at the END of the call -- nothing is
@@ -672,6 +686,370 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));
     NF_CUDA_OK(cudaStreamSynchronize(st));
     if (sc[0]) { set_error("nf_bin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
+    p->n_units = (long long)sc[2];
+    p->have_bin_time = true;
+    p->launches_bin = L;
+    return NF_OK;
+}
+
+
+// ==================================================================================================================
+// Incremental re-binning (nf_rebin).  The paper's pipeline moves particles to their new cells
+// after every drift ("reorders particles into their new cells"; "moving particles to their new cells",
+// PAPER.md:353; Table 6 "Finish" / "Merge New Particles"), and a particle drifts much less than a
+// cell per step, so almost every particle STAYS in its cell.  Result (cid, count, offset, perm, source arrays, units):
+// exactly what nf_bin gives for the new positions -- the stable order inside a cell is ascending input index, so the
+// new order of a cell is the merge of its stayers (already ascending in the old order) with its arrivals:
+//     new slot of a stayer at old slot s, cell c, index i  =  G(s) + arr_off[c] + #{arrivals of c with index < i}
+//     new slot of an arrival (c, i)                        =  arr_off[c] + #{arrivals of c with index < i} + G(s*)
+// with G(s) = stayers among the old slots below s, arr_off = exclusive scan of the arrivals per cell, s* = first old
+// slot of cell c whose index is >= i (or the end of the cell).  No radix pass: one pass over the input order (cell ids,
+// movers), one pass over the old sorted order (G by a decoupled look-back, perm, gather into the source arrays).
+__device__ __forceinline__ uint32_t cell_of(const float *p3, const Consts &k, bool &bad)
+{
+    int c[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        const double x = (double)p3[d];
+        if (!(x >= 0.0 && x < k.L)) bad = true;
+        int q = (int)floor(x * k.inv_cell_w);
+        q = q >= k.cpd ? k.cpd - 1 : (q < 0 ? 0 : q);
+        c[d] = q;
+    }
+    return ((uint32_t)c[0] * k.cpd + c[1]) * k.cpd + c[2];
+}
+
+// pass 1, input order: new cell ids (reading C6), movers, count deltas, arrivals per cell.  A thread takes 4 consecutive
+// particles: 48 contiguous bytes of positions as three 16-byte loads, the four old ids as one.
+__global__ void __launch_bounds__(256) rebin_cellid_kernel(const float *__restrict__ pos, size_t n, Consts k, uint32_t *__restrict__ cid,
+                                                           uint32_t *__restrict__ count, uint32_t *__restrict__ arr_count,
+                                                           uint32_t *__restrict__ mover_list, uint32_t cap,
+                                                           uint32_t *__restrict__ moverbits, uint32_t *__restrict__ scalars, int vec)
+{
+    __shared__ uint32_t s_cnt, s_base;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    const size_t i0 = ((size_t)blockIdx.x * 256 + threadIdx.x) * 4;
+    bool bad = false;
+    uint32_t moved = 0;                                // bit j: particle i0 + j changed its cell
+    uint32_t id[4] = {0, 0, 0, 0};
+    if (vec && i0 + 4 <= n) {                          // vec: the caller's array is 16-byte aligned
+        const float4 *p4 = reinterpret_cast<const float4 *>(pos + 3 * i0);           // 3 i0 floats = 48 (i0 / 4) bytes: 16-byte aligned
+        const float4 v0 = __ldg(p4), v1 = __ldg(p4 + 1), v2 = __ldg(p4 + 2);
+        const uint4 old = *reinterpret_cast<const uint4 *>(cid + i0);
+        const float c[12] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w, v2.x, v2.y, v2.z, v2.w};
+        const uint32_t o[4] = {old.x, old.y, old.z, old.w};
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            id[j] = cell_of(c + 3 * j, k, bad);
+            if (id[j] != o[j]) { moved |= 1u << j; atomicSub(&count[o[j]], 1u); }
+        }
+    } else {
+        for (int j = 0; j < 4 && i0 + j < n; j++) {
+            id[j] = cell_of(pos + 3 * (i0 + j), k, bad);
+            const uint32_t old = cid[i0 + j];
+            if (id[j] != old) { moved |= 1u << j; atomicSub(&count[old], 1u); }
+        }
+    }
+    // the block reserves its share of the mover list with ONE global atomic (every mover adding to the same counter
+    // serialises in L2: 160 000 movers cost 80 us that way)
+    uint32_t local = 0;
+    if (moved) local = atomicAdd(&s_cnt, (uint32_t)__popc(moved));
+    __syncthreads();
+    if (threadIdx.x == 0 && s_cnt) s_base = atomicAdd(&scalars[4], s_cnt);
+    __syncthreads();
+    if (moved) {
+        uint32_t q = s_base + local;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            if ((moved >> j) & 1u) {
+                cid[i0 + j] = id[j];
+                atomicAdd(&count[id[j]], 1u);
+                atomicAdd(&arr_count[id[j]], 1u);
+                if (q < cap) mover_list[q] = (uint32_t)(i0 + j);
+                q++;
+            }
+        }
+    }
+    // 8 threads make one 32-bit word of the mover bitmap
+    uint32_t word = moved << (4 * (threadIdx.x & 7));
+    word |= __shfl_xor_sync(0xffffffffu, word, 1);
+    word |= __shfl_xor_sync(0xffffffffu, word, 2);
+    word |= __shfl_xor_sync(0xffffffffu, word, 4);
+    if ((threadIdx.x & 7) == 0 && i0 < n) moverbits[i0 >> 5] = word;
+    if (bad) atomicOr(&scalars[0], 1u);
+}
+
+// the movers grouped by their new cell (unordered inside a cell: the lists are short)
+__global__ void __launch_bounds__(256) rebin_fill_kernel(const uint32_t *__restrict__ mover_list, uint32_t cap, const uint32_t *__restrict__ scalars,
+                                                         const uint32_t *__restrict__ cid, const uint32_t *__restrict__ arr_off,
+                                                         uint32_t *__restrict__ arr_cursor, uint32_t *__restrict__ arr_list)
+{
+    const uint32_t q = blockIdx.x * 256 + threadIdx.x;
+    const uint32_t m = min(scalars[4], cap);
+    if (q >= m) return;
+    const uint32_t i = mover_list[q], c = cid[i];
+    const uint32_t at = arr_off[c] + atomicAdd(&arr_cursor[c], 1u);
+    if (at < cap) arr_list[at] = i;
+}
+
+// sum over the cells of (arrivals)^2: the ranking below compares every arrival of a cell with every other one
+__global__ void __launch_bounds__(256) rebin_work_kernel(const uint32_t *__restrict__ arr_count, uint32_t ncells, unsigned long long *__restrict__ work)
+{
+    const uint32_t c = blockIdx.x * 256 + threadIdx.x;
+    unsigned long long w = c < ncells ? (unsigned long long)arr_count[c] * arr_count[c] : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) w += __shfl_down_sync(0xffffffffu, w, o);
+    if ((threadIdx.x & 31) == 0 && w) atomicAdd(work, w);
+}
+
+// every cell's arrivals in ascending input index (the stable order): rank by comparison inside the (short) list
+__global__ void __launch_bounds__(256) rebin_rank_kernel(const uint32_t *__restrict__ arr_list, uint32_t cap, uint32_t *__restrict__ scalars,
+                                                         const unsigned long long *__restrict__ work, unsigned long long budget,
+                                                         const uint32_t *__restrict__ cid, const uint32_t *__restrict__ arr_off,
+                                                         const uint32_t *__restrict__ arr_count, uint32_t *__restrict__ arr_sorted)
+{
+    const uint32_t q = blockIdx.x * 256 + threadIdx.x;
+    const uint32_t movers = scalars[4];
+    if (movers > cap || *work > budget) { if (q == 0) atomicOr(&scalars[5], 1u); return; }
+    if (q >= movers) return;
+    const uint32_t i = arr_list[q], c = cid[i];
+    const uint32_t a0 = arr_off[c], ac = arr_count[c];
+    uint32_t rank = 0;
+    for (uint32_t j = 0; j < ac; j++) rank += __ldg(arr_list + a0 + j) < i;
+    arr_sorted[a0 + rank] = i;
+}
+
+// cell of every sorted slot (once after a full nf_bin; nf_rebin keeps it up to date afterwards)
+__global__ void __launch_bounds__(256) slotcell_kernel(const uint32_t *__restrict__ offset, uint32_t ncells, size_t n, uint32_t *__restrict__ slotcell)
+{
+    const size_t s = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (s >= n) return;
+    uint32_t lo = 0, hi = ncells;                      // last c with offset[c] <= s
+    while (lo + 1 < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (__ldg(offset + mid) <= (uint32_t)s) lo = mid; else hi = mid;
+    }
+    slotcell[s] = lo;
+}
+
+struct RebinArgs {
+    const float *pos;
+    const uint32_t *perm_old, *slotcell_old, *cid, *moverbits, *arr_off, *arr_count, *arr_list, *offset_old, *offset_new, *poff;
+    uint32_t *perm_new, *slotcell_new, *staybits, *wordprefix, *scalars;
+    unsigned long long *tile_state;
+    float *X, *Y, *Z;
+    Consts k;
+    size_t n;
+    uint32_t cap;
+};
+
+// writes particle i (cell c, new sorted slot dst) into the padded SoA source arrays, with the pads after the cell's last particle
+__device__ __forceinline__ void rebin_store(const RebinArgs &a, uint32_t c, uint32_t dst, float x, float y, float z)
+{
+    const Consts &k = a.k;
+    const float sc = (float)k.scale;
+    const uint32_t cz = c % k.cpd, cy = (c / k.cpd) % k.cpd, cx = c / (k.cpd * k.cpd);
+    const float ox = (float)((double)cx * k.cell_w), oy = (float)((double)cy * k.cell_w), oz = (float)((double)cz * k.cell_w);
+    const uint32_t o0 = a.offset_new[c], o1 = a.offset_new[c + 1];
+    const uint32_t p = a.poff[c] + (dst - o0);
+    a.X[p] = (x - ox) * sc;
+    a.Y[p] = (y - oy) * sc;
+    a.Z[p] = (z - oz) * sc;
+    if (dst + 1 == o1) {
+        const uint32_t pe = a.poff[c + 1];
+        for (uint32_t q = p + 1; q < pe; q++) { a.X[q] = kDummy; a.Y[q] = kDummy; a.Z[q] = kDummy; }
+    }
+}
+
+// pass 2, old sorted order: one block per tile of kSortTile slots, tiles taken in ticket order (look-back needs the
+// earlier tiles to be running).  Each warp owns 512 consecutive slots, 32 per round: a round's ballot IS the stay word.
+__global__ void __launch_bounds__(kSortThreads, 2) rebin_merge_kernel(const RebinArgs a)
+{
+    __shared__ uint32_t s_tile, s_base;
+    __shared__ uint32_t s_warp[kSortWarps];
+    __shared__ float s_xyz[kSortWarps][96];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_tile = atomicAdd(&a.scalars[6], 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const size_t tile0 = (size_t)tile * kSortTile, n = a.n;
+    if (tile0 >= n) return;
+    if (a.scalars[5]) return;                          // more movers than the merge handles: the host sorts from scratch
+    const size_t seg = tile0 + (size_t)w * (32 * kSortItems);
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t idx[kSortItems], cell[kSortItems], wd[kSortItems];
+    uint32_t wtot = 0;
+#pragma unroll
+    for (int r = 0; r < kSortItems; r++) {
+        const size_t e = seg + r * 32 + lane;
+        const bool valid = e < n;
+        idx[r] = valid ? a.perm_old[e] : 0u;
+        cell[r] = valid ? a.slotcell_old[e] : 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < kSortItems; r++) {
+        const size_t e = seg + r * 32 + lane;
+        const bool stay = e < n && !((__ldg(a.moverbits + (idx[r] >> 5)) >> (idx[r] & 31u)) & 1u);
+        wd[r] = __ballot_sync(0xffffffffu, stay);
+        wtot += __popc(wd[r]);
+        if (lane == 0 && seg + r * 32 < n) a.staybits[(seg + r * 32) >> 5] = wd[r];
+    }
+    if (lane == 0) s_warp[w] = wtot;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (int q = 0; q < kSortWarps; q++) { const uint32_t t = s_warp[q]; s_warp[q] = run; run += t; }
+        // decoupled look-back over the tiles: state = flag << 32 | value; flag 1: the tile's own count, 2: inclusive prefix
+        volatile unsigned long long *st = a.tile_state;
+        uint32_t base = 0;
+        if (tile > 0) {
+            st[tile] = (1ull << 32) | run;
+            for (int t = (int)tile - 1;; t--) {
+                unsigned long long v;
+                do { v = st[t]; } while ((v >> 32) == 0ull);
+                base += (uint32_t)v;
+                if ((v >> 32) == 2ull) break;
+            }
+        }
+        st[tile] = (2ull << 32) | (unsigned long long)(base + run);
+        s_base = base;
+    }
+    __syncthreads();
+    uint32_t run = s_base + s_warp[w];
+    // the warp's three loads of a round: adjacent lanes read adjacent floats of one particle (12-byte gathers touch ~14
+    // sectors per request instead of 32), handed to the owning lanes through shared memory
+    auto fetch = [&](const uint32_t idr, const uint32_t wdr, float (&f)[3]) {
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            const uint32_t flat = j * 32 + lane, q = flat / 3u, comp = flat - 3u * q;
+            const uint32_t iq = __shfl_sync(0xffffffffu, idr, q);
+            f[j] = ((wdr >> q) & 1u) ? __ldg(a.pos + 3 * (size_t)iq + comp) : 0.f;
+        }
+    };
+    constexpr int kAhead = 4;                          // rounds whose gathers are in flight together
+#pragma unroll
+    for (int r0 = 0; r0 < kSortItems; r0 += kAhead) {
+        if (seg + r0 * 32 >= n) break;                 // warp-uniform
+        float f[kAhead][3];
+#pragma unroll
+        for (int g = 0; g < kAhead; g++) fetch(idx[r0 + g], wd[r0 + g], f[g]);
+#pragma unroll
+        for (int g = 0; g < kAhead; g++) {
+            const int r = r0 + g;
+            if (seg + r * 32 >= n) break;
+            if (lane == 0) a.wordprefix[(seg + r * 32) >> 5] = run;
+#pragma unroll
+            for (int j = 0; j < 3; j++) s_xyz[w][j * 32 + lane] = f[g][j];
+            __syncwarp();
+            if ((wd[r] >> lane) & 1u) {
+                const uint32_t i = idx[r], c = cell[r];
+                const uint32_t ac = __ldg(a.arr_count + c), a0 = __ldg(a.arr_off + c);
+                uint32_t lo = 0, hi = ac;              // arrivals of the cell with a smaller index (the list is ascending)
+                while (lo < hi) {
+                    const uint32_t mid = (lo + hi) >> 1;
+                    if (__ldg(a.arr_list + a0 + mid) < i) lo = mid + 1; else hi = mid;
+                }
+                const uint32_t dst = run + __popc(wd[r] & lt) + a0 + lo;
+                a.perm_new[dst] = i;
+                a.slotcell_new[dst] = c;
+                rebin_store(a, c, dst, s_xyz[w][3 * lane + 0], s_xyz[w][3 * lane + 1], s_xyz[w][3 * lane + 2]);
+            }
+            __syncwarp();
+            run += __popc(wd[r]);
+        }
+    }
+}
+
+// pass 2b: the arrivals
+__global__ void __launch_bounds__(256) rebin_arrivals_kernel(const RebinArgs a)
+{
+    const uint32_t q = blockIdx.x * 256 + threadIdx.x;
+    const uint32_t movers = a.scalars[4];
+    if (a.scalars[5] || q >= movers) return;
+    const uint32_t i = a.arr_list[q], c = a.cid[i];
+    const uint32_t a0 = a.arr_off[c], rank = q - a0;               // the lists are sorted: the position is the rank
+    uint32_t lo = a.offset_old[c], hi = a.offset_old[c + 1];       // first old slot of cell c with index >= i
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (a.perm_old[mid] < i) lo = mid + 1; else hi = mid;
+    }
+    const uint32_t stayers_below = (size_t)lo < a.n ? a.wordprefix[lo >> 5] + __popc(a.staybits[lo >> 5] & ((1u << (lo & 31u)) - 1u))
+                                                    : (uint32_t)a.n - movers;
+    const uint32_t dst = a0 + rank + stayers_below;
+    a.perm_new[dst] = i;
+    a.slotcell_new[dst] = c;
+    const float *p3 = a.pos + 3 * (size_t)i;
+    rebin_store(a, c, dst, p3[0], p3[1], p3[2]);
+}
+
+int launch_rebin(nf_plan *p, const float *pos)
+{
+    const size_t n = (size_t)p->n;
+    const Consts &k = p->k;
+    Workspace &ws = p->ws;
+    cudaStream_t st = p->stream;
+    // particles that changed cell in the previous call: above 1/16 of them the merge costs more than the sort
+    if (p->rebin_movers > (long long)(n / 16)) {
+        p->rebin_movers = -1; p->rebin_path = 2;
+        return launch_bin(p, pos, p->n);
+    }
+    int L = 0;
+    p->have_bin_time = false;
+    p->n_units = 0;
+    const uint32_t cap = (uint32_t)(n / 4 + 32);
+    const uint32_t *perm_old = p->perm;
+    uint32_t *perm_new = perm_old == ws.valA ? ws.valB : ws.valA;
+    NF_CUDA_OK(cudaEventRecord(p->ev[0], st));
+    if (!p->slotcell) {
+        slotcell_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(ws.offset, k.ncells, n, ws.keyA);  L++;
+        p->slotcell = ws.keyA;
+    }
+    const uint32_t *slotcell_old = p->slotcell;
+    uint32_t *slotcell_new = slotcell_old == ws.keyA ? ws.keyB : ws.keyA;
+    NF_CUDA_OK(cudaMemsetAsync(ws.scalars, 0, 4 * 64, st));
+    NF_CUDA_OK(cudaMemsetAsync(ws.interactions, 0, 16, st));
+    NF_CUDA_OK(cudaMemsetAsync(ws.arr_count, 0, 4 * (size_t)(k.ncells + 1), st));
+    NF_CUDA_OK(cudaMemsetAsync(ws.arr_cursor, 0, 4 * (size_t)(k.ncells + 1), st));
+    const size_t ntiles = (n + kSortTile - 1) / kSortTile;
+    NF_CUDA_OK(cudaMemsetAsync(ws.tile_state, 0, 8 * (ntiles + 1), st));
+    rebin_cellid_kernel<<<(unsigned)((n + 1023) / 1024), 256, 0, st>>>(pos, n, k, ws.cid, ws.count, ws.arr_count, ws.mover_list, cap,
+                                                                     ws.moverbits, ws.scalars, ((uintptr_t)pos & 15) == 0);  L++;
+    exclusive_scan(ws.arr_count, ws.arr_off, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
+    exclusive_scan(ws.count, ws.offset_new, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
+    exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
+    rebin_fill_kernel<<<(cap + 255) / 256, 256, 0, st>>>(ws.mover_list, cap, ws.scalars, ws.cid, ws.arr_off, ws.arr_cursor, ws.arr_list);  L++;
+    // the cells' arrival lists in ascending index: ranked by comparison, sum of (arrivals per cell)^2 operations, bounded by
+    // 16 n (a 3e6-particle halo cell that exchanges 1 % of its members costs 9e8); beyond that the host sorts from scratch
+    rebin_work_kernel<<<(k.ncells + 255) / 256, 256, 0, st>>>(ws.arr_count, k.ncells, ws.interactions + 1);  L++;
+    rebin_rank_kernel<<<(cap + 255) / 256, 256, 0, st>>>(ws.arr_list, cap, ws.scalars, ws.interactions + 1, 16ull * n + 4096, ws.cid,
+                                                         ws.arr_off, ws.arr_count, ws.mover_list);  L++;
+    RebinArgs a;
+    a.pos = pos; a.perm_old = perm_old; a.slotcell_old = slotcell_old; a.cid = ws.cid; a.moverbits = ws.moverbits;
+    a.arr_off = ws.arr_off; a.arr_count = ws.arr_count; a.arr_list = ws.mover_list;      // sorted lists (the mover list's storage)
+    a.offset_old = ws.offset; a.offset_new = ws.offset_new; a.poff = ws.poff;
+    a.perm_new = perm_new; a.slotcell_new = slotcell_new; a.staybits = ws.staybits; a.wordprefix = ws.wordprefix;
+    a.scalars = ws.scalars; a.tile_state = ws.tile_state; a.X = ws.x; a.Y = ws.y; a.Z = ws.z; a.k = k; a.n = n; a.cap = cap;
+    rebin_merge_kernel<<<(unsigned)ntiles, kSortThreads, 0, st>>>(a);  L++;
+    rebin_arrivals_kernel<<<(cap + 255) / 256, 256, 0, st>>>(a);  L++;
+    NF_CUDA_OK(cudaGetLastError());
+    NF_CUDA_OK(cudaMemcpyAsync(ws.offset, ws.offset_new, 4 * (size_t)(k.ncells + 1), cudaMemcpyDeviceToDevice, st));
+    p->perm = perm_new;
+    p->slotcell = slotcell_new;
+    // the old perm / slot-cell arrays are free now: scratch of the unit sort
+    { const int rc = launch_units(p, n, const_cast<uint32_t *>(slotcell_old), const_cast<uint32_t *>(perm_old), &L); if (rc != NF_OK) return rc; }
+    NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
+    NF_CUDA_OK(cudaGetLastError());
+    uint32_t sc[8];
+    NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));   // the call's one synchronisation, at its end
+    NF_CUDA_OK(cudaStreamSynchronize(st));
+    if (sc[0]) { set_error("nf_rebin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
+    p->rebin_movers = (long long)sc[4];
+    if (sc[5] || sc[4] > cap) {                       // more movers (or arrivals into one cell) than the merge handles: sort from scratch
+        p->rebin_path = 2;
+        return launch_bin(p, pos, p->n);
+    }
+    p->rebin_path = 1;
     p->n_units = (long long)sc[2];
     p->have_bin_time = true;
     p->launches_bin = L;

@@ -78,7 +78,15 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
     Unit *units, *units_sorted;                   // [U_max]
     uint32_t *bucket_hist;                        // [64] + cursor
     unsigned long long *interactions;             // [1]
-    uint32_t *scalars;                            // [16]: 0 error flag, 1 unit counter, 2 n_units, 3 padded total
+    uint32_t *scalars;                            // [64]: 0 error flag, 1 unit counter, 2 n_units, 3 padded total,
+                                                  //       4 movers of the last nf_rebin, 5 rebin fallback flag, 6 look-back ticket
+    // incremental re-binning (nf_rebin)
+    uint32_t *offset_new;                         // [C+2]
+    uint32_t *arr_count, *arr_off, *arr_cursor;   // [C+2] arrivals per cell, their exclusive scan, fill cursors
+    uint32_t *mover_list, *arr_list;              // [n/4 + 64] input indices of the movers; the same grouped by new cell
+    uint32_t *moverbits;                          // [n/32 + 2] bit i: particle i changed its cell
+    uint32_t *staybits, *wordprefix;              // [n/32 + 2] by OLD sorted slot: stays in its cell; stayers before the word
+    unsigned long long *tile_state;               // [n/8192 + 2] decoupled look-back of the merge pass
     size_t bytes;
 };
 
@@ -116,6 +124,9 @@ struct nf_plan {
     long long n_units;
     int sort_passes;
     const uint32_t *perm;
+    const uint32_t *slotcell;       // cell of every sorted slot (nf_rebin keeps it; NULL after a full nf_bin until first needed)
+    long long rebin_movers;         // particles that changed cell in the last nf_rebin (-1: unknown)
+    int rebin_path;                 // 0: none yet, 1: incremental, 2: full sort
     // optional source masses (nf_set_masses): padded SoA like ws.x, plan-owned, outside the arena
     float *mass_soa; size_t mass_cap; bool have_mass;
     // host-buffer path
@@ -132,6 +143,7 @@ namespace nf {
 void set_error(const char *fmt, ...);
 size_t carve(Workspace &ws, void *base, long long n, int cpd);   // base may be NULL (size only)
 int  launch_bin(nf_plan *p, const float *pos, long long n);             // S1-S5 (nf_bin.cu)
+int  launch_rebin(nf_plan *p, const float *pos);                        // S1-S5 for moved particles of the same set (nf_bin.cu)
 int  launch_set_masses(nf_plan *p, const float *mass);                  // masses of the binned particles -> padded SoA (nf_bin.cu)
 int  launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, double dt, float *amax_cell);   // S6-S7 (nf_direct.cu)
 int  accel_max_ctas_per_sm(int variant);

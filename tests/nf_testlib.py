@@ -15,7 +15,7 @@ TOL_MAX = 1e-3    # ... and at the maximum
 # The first three are worst cases per term, the last is the random walk of the chain; measured worst ratios are printed
 # at the end of the run (conftest.py) and recorded in DESIGN.md 5.
 C13 = 2.0e-6
-RATIOS = []       # (what, worst |err| / S over rows that miss the 1e-5 rule) -- reported by conftest.py
+RATIOS = []       # (what, worst |err| / S over the rows that miss the 1e-5 rule, their number, rows, worst |err| / S of all rows)
 
 
 def u32(t: torch.Tensor) -> np.ndarray:
@@ -70,8 +70,9 @@ def assert_parity_conditioned(a_gpu, a_ref, scale, what=""):
     loose = (err <= TOL_MAX * den) | cond
     ratio = err / np.where(scale > 0, scale, 1.0)
     ratio[(scale == 0) & (err == 0)] = 0.0
-    worst = float(ratio.max())
-    RATIOS.append((what, worst, int((~(err <= TOL_P999 * den)).sum()), len(err)))
+    on_c13 = ~(err <= TOL_P999 * den)                   # rows BASELINE.json's 1e-5 does not cover: judged by C13 x S
+    worst = float(ratio[on_c13].max()) if on_c13.any() else 0.0
+    RATIOS.append((what, worst, int(on_c13.sum()), len(err), float(ratio.max())))
     assert tight.mean() >= 0.999, (f"{what}: {(~tight).sum()} of {len(err)} rows miss both 1e-5 |a_ref| and C13 S "
                                    f"(worst err/S {worst:.3e})")
     assert loose.all(), f"{what}: {(~loose).sum()} rows miss both 1e-3 |a_ref| and C13 S (worst err/S {worst:.3e})"

@@ -821,3 +821,170 @@ def test_short_windows_share_stages(oracle_mod, ns):
     assert_parity(a1.numpy().astype(np.float64), ref, f"column of {ns}")
     rho_ref = oracle_mod.density(pos.numpy(), cpd, L, 0.05, R)
     assert np.all(np.abs(rho.cpu().numpy() - rho_ref) <= 1e-5 * rho_ref)
+
+
+# ---------------------------------------------------------------- incremental re-binning (nf_rebin)
+def _drift(pos: torch.Tensor, L: float, cell: float, rms_cells: float, gen: torch.Generator, jump_frac: float = 0.0):
+    """Seeded sub-cell displacements (the paper's particles drift much less than a cell per step), wrapped
+    through the periodic faces; `jump_frac` of the particles additionally jump by up to two cells."""
+    d = torch.randn(pos.shape, generator=gen, dtype=torch.float64) * (rms_cells * cell)
+    if jump_frac > 0:
+        who = torch.rand(pos.shape[0], generator=gen) < jump_frac
+        d[who] += (torch.rand((int(who.sum()), 3), generator=gen, dtype=torch.float64) - 0.5) * 4 * cell
+    q = torch.remainder(pos.double() + d, L).to(torch.float32)
+    q[q >= L] = 0.0
+    return q.contiguous()
+
+
+def _rebin_check(oracle_mod, plan, pos, cfg, what, expect_path=None, fresh=True):
+    import paper_2110_11398_b200 as nf
+    plan.rebin(pos.cuda())
+    acc = plan.accel()
+    torch.cuda.synchronize()
+    st = plan.stats()
+    b = oracle_mod.bin_particles(pos.numpy(), cfg.cpd, cfg.L)
+    assert_binning_equal({k: u32(v) for k, v in plan.binning().items()}, b)          # byte-equal to the oracle's definition
+    assert st["interactions"] == oracle_mod.interactions(b["count"], cfg.cpd, cfg.R), what
+    if expect_path is not None:
+        assert st["rebin_path"] == expect_path, (what, st["rebin_path"], st["rebin_movers"])
+    if fresh:                                                                       # same layout => same bits as a full nf_bin
+        with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p2:
+            p2.bin(pos.cuda())
+            acc2 = p2.accel()
+            lay, lay2 = plan.layout(), p2.layout()
+            for key in ("poff", "x", "y", "z"):
+                assert torch.equal(lay[key], lay2[key]), (what, key)
+            assert torch.equal(acc, acc2), what
+    return acc, b, st
+
+
+@pytest.mark.parametrize("idx,n_side,cpd", [(3, 40, 10), (4, 40, 10), (2, 48, 12), (1, 32, 9)])
+def test_rebin_drift_steps(oracle_mod, idx, n_side, cpd):
+    """k drift steps of seeded sub-cell displacements (face crossings, the periodic boundary, particles leaving the heavy
+    cells of the clustered recipe): after every step nf_rebin equals nfo_bin byte for byte and the accelerations meet the
+    tolerance (and are bit-identical to those of a fresh nf_bin)."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.scaled(idx, n_side, cpd)
+    pos = nf_inputs.generate(cfg)
+    gen = torch.Generator().manual_seed(900 + idx)
+    cell = cfg.L / cfg.cpd
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos.cuda())
+        prev, seen = 0, 0
+        for step, (rms, jump) in enumerate([(0.004, 0.0), (0.01, 0.0), (0.0, 0.0), (0.02, 0.002), (0.1, 0.0), (0.004, 0.0), (0.004, 0.0)]):
+            pos = _drift(pos, cfg.L, cell, rms, gen, jump) if rms > 0 or jump > 0 else pos
+            # more than 1/16 of the particles moved in the previous call: this one sorts from scratch (and counts no movers)
+            # (a large drift may also overflow the per-cell arrival lists of the halo cells: either path is right then)
+            path = 2 if prev > cfg.n // 16 else (None if rms >= 0.05 else 1)
+            acc, b, st = _rebin_check(oracle_mod, plan, pos, cfg, f"{cfg.name} drift step {step}", expect_path=path)
+            prev = st["rebin_movers"]
+            if path == 1 and step == 2:
+                assert st["rebin_movers"] == 0
+            elif path == 1:
+                assert 0 <= st["rebin_movers"] < cfg.n // 4
+                seen += st["rebin_movers"]
+            ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R, binning=b)
+            assert_parity(acc.cpu().numpy().astype(np.float64), ref, f"{cfg.name} drift step {step}")
+        assert seen > 0                                                # the merge path really moved particles
+
+
+def test_rebin_fallbacks_and_errors(oracle_mod):
+    """Everything moved (new random positions), one cell receiving more arrivals than the merge handles, the call after
+    a step with many movers, errors: the result is always nfo_bin's."""
+    import paper_2110_11398_b200 as nf
+    B = nf.binding
+    cfg = nf_inputs.scaled(3, 32, 8)
+    pos = nf_inputs.generate(cfg)
+    gen = torch.Generator().manual_seed(77)
+    cell = cfg.L / cfg.cpd
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        with pytest.raises(nf.NFError) as e:
+            plan.rebin(pos.cuda())
+        assert e.value.code == B.NF_ERR_STATE
+        plan.bin(pos.cuda())
+        with pytest.raises(ValueError):
+            plan.rebin(pos[:100].cuda())                                   # another n: the binding refuses
+        pos = torch.rand(pos.shape, generator=gen)                         # every particle somewhere else: sorted from scratch
+        _rebin_check(oracle_mod, plan, pos, cfg, "teleport", expect_path=2)
+        pos = _drift(pos, cfg.L, cell, 0.3, gen)                           # ~1/3 of the particles change cell: merge still exact
+        _, _, st = _rebin_check(oracle_mod, plan, pos, cfg, "large drift")
+        pos = _drift(pos, cfg.L, cell, 0.01, gen)                          # the call after many movers goes straight to the sort
+        _rebin_check(oracle_mod, plan, pos, cfg, "after many movers", expect_path=2 if st["rebin_movers"] > cfg.n // 16 else 1)
+        pos = _drift(pos, cfg.L, cell, 0.01, gen)
+        _rebin_check(oracle_mod, plan, pos, cfg, "incremental again", expect_path=1)
+        q = pos.clone()                                                    # 2000 particles collapse into one cell (> 512 arrivals)
+        q[:2000] = torch.tensor([0.51, 0.52, 0.53]) + torch.rand((2000, 3), generator=gen) * 0.01
+        _rebin_check(oracle_mod, plan, q.contiguous(), cfg, "collapse into one cell", expect_path=2)
+        bad = q.clone()
+        bad[5, 1] = float("nan")
+        with pytest.raises(nf.NFError) as e:
+            plan.rebin(bad.cuda())
+        assert e.value.code == B.NF_ERR_DOMAIN
+        with pytest.raises(nf.NFError) as e:                               # the binning is invalid after the error
+            plan.accel()
+        assert e.value.code == B.NF_ERR_STATE
+        plan.bin(q.cuda())
+        plan.set_sink_slabs(1, 3)                                          # options that change the units need a fresh nf_bin
+        with pytest.raises(nf.NFError) as e:
+            plan.rebin(q.cuda())
+        assert e.value.code == B.NF_ERR_STATE
+    with nf.Plan(5, 1.0, 0.01, 2) as plan:                                 # one particle, and none
+        one = torch.tensor([[0.999, 0.5, 0.001]])
+        plan.bin(one.cuda())
+        plan.rebin(torch.tensor([[0.001, 0.5, 0.999]]).cuda())
+        assert u32(plan.binning()["cid"]).tolist() == [0 * 25 + 2 * 5 + 4]
+        assert torch.all(plan.accel() == 0)
+        plan.bin(torch.empty((0, 3)).cuda())
+        plan.rebin(torch.empty((0, 3)).cuda())
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_rebin_fuzz(oracle_mod, seed):
+    """Random grids, distributions and drift amplitudes (none, tiny, a third of a cell, several cells), slab-restricted
+    sinks, both kernel variants: three steps each against the oracle's binning, bit-identical to a fresh nf_bin."""
+    import paper_2110_11398_b200 as nf
+    from test_gpu_fuzz import KINDS, _positions
+    rng = np.random.default_rng(4200 + seed)
+    R = int(rng.integers(0, 4))
+    cpd = int(rng.integers(2 * R + 1, 2 * R + 1 + rng.choice([1, 6, 20])))
+    L = float(rng.choice([1.0, 0.125, 7.5]))
+    n = int(rng.choice([1, 33, 3000, 20000, 60000]))
+    pos = torch.from_numpy(_positions(rng, KINDS[seed % len(KINDS)], n, L))
+    cell = L / cpd
+    gen = torch.Generator().manual_seed(seed)
+    with nf.Plan(cpd, L, 0.02 * cell, R) as plan:
+        plan.set_option("variant", int(rng.integers(0, 2)))
+        plan.bin(pos.cuda())
+        for step in range(3):
+            rms = float(rng.choice([0.0, 0.003, 0.03, 0.3, 1.5]))
+            pos = _drift(pos, L, cell, rms, gen, jump_frac=float(rng.choice([0.0, 0.01])))
+            plan.rebin(pos.cuda())
+            acc = plan.accel()
+            b = oracle_mod.bin_particles(pos.numpy(), cpd, L)
+            assert_binning_equal({k: u32(v) for k, v in plan.binning().items()}, b)
+            with nf.Plan(cpd, L, 0.02 * cell, R) as p2:
+                p2.set_option("variant", 0)
+                p2.bin(pos.cuda())
+                lay, lay2 = plan.layout(), p2.layout()
+                for key in ("poff", "x", "y", "z"):
+                    assert torch.equal(lay[key], lay2[key]), (seed, step, key)
+            assert plan.stats()["interactions"] == oracle_mod.interactions(b["count"], cpd, R)
+            assert torch.isfinite(acc).all()
+
+
+@pytest.mark.parametrize("idx,device", [(3, "cpu"), (4, "cuda")])
+def test_rebin_full_size(oracle_mod, idx, device):
+    """Config 3 / config 4 size: two drift steps at ~1 % movers, byte-equal to nfo_bin; prints the time of both paths."""
+    import paper_2110_11398_b200 as nf
+    cfg = nf_inputs.config(idx)
+    pos = nf_inputs.generate(cfg, device=device).cpu()
+    gen = torch.Generator().manual_seed(31 + idx)
+    cell = cfg.L / cfg.cpd
+    with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
+        plan.bin(pos.cuda())
+        ms_full = plan.stats()["ms_bin"]
+        for step in range(2):
+            pos = _drift(pos, cfg.L, cell, 0.004, gen)
+            _, b, st = _rebin_check(oracle_mod, plan, pos, cfg, f"{cfg.name} rebin {step}", expect_path=1, fresh=(step == 1))
+            print(f"{cfg.name}: nf_bin {ms_full:.3f} ms, nf_rebin {st['ms_bin']:.3f} ms with {st['rebin_movers']} movers "
+                  f"({100.0 * st['rebin_movers'] / cfg.n:.2f} %)")

@@ -452,18 +452,25 @@ def main_slabs(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = nf_inputs.config(args.config)
     pos = nf_inputs.generate(cfg, device="cuda" if cfg.n > 20_000_000 else "cpu").cuda()   # same seed on every rank
-    first, cnt = slabs.slab_partition(cfg.cpd, world)[rank]
-    own = pos[((slabs.slab_of(pos, cfg.cpd, cfg.L) - first) % cfg.cpd) < cnt].contiguous()
-    del pos
-    torch.cuda.empty_cache()
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
         apply_options(plan, args)
+        # set-up (outside the timed region): the scheduler's exact pair-interaction count per slab of the whole box gives
+        # the cost-balanced contiguous ranges (nf_get_slab_cost + nf_slab_partition; in a running simulation the ranks
+        # all-reduce the vectors of their own slabs from the previous step); the rank's particles are selected on the device
+        plan.bin(pos)
+        parts = slabs.slab_partition(cfg.cpd, world, plan.slab_cost())
+        first, cnt = parts[rank]
+        own, _ = plan.slab_select(pos, first, cnt, pos.shape[0])
+        own = own.contiguous()
+        del pos
+        torch.cuda.empty_cache()
         plan.set_sink_slabs(first, cnt)
+        sel = slabs.LibrarySelector(plan)
         acc = None
 
         def step():
             nonlocal acc
-            loc, n_own = slabs.halo_exchange(own, cfg.cpd, cfg.L, cfg.R, rank, world, dist)
+            loc, n_own = slabs.halo_exchange(own, cfg.cpd, cfg.R, rank, world, parts, dist, sel)
             if acc is None or acc.shape[0] != loc.shape[0]:
                 acc = torch.empty_like(loc)
             plan.bin(loc)
@@ -498,7 +505,8 @@ def main_slabs(args):
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": cfg.name, "n": n, "cpd": cfg.cpd, "R": cfg.R, "eps": cfg.eps, "L": cfg.L,
                            "interactions_per_step": I, "l2": "inputs exceed L2",
-                           "parallelism": f"x-slabs dp{world}, R-slab halo exchange every step (torch.distributed P2P over NCCL)",
+                           "parallelism": f"x-slabs dp{world}, cost-balanced ranges {parts}, R-slab halo packed on the device "
+                                          "(nf_slab_select) and exchanged every step (torch.distributed P2P over NCCL)",
                            "rank0_local_particles": n_local},
                 "particle_updates_per_s": n * args.steps / (t_total / 1e3),
                 "gpu_launches": args.steps * (st["kernel_launches_bin"] + st["kernel_launches_accel"]),

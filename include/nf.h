@@ -181,6 +181,32 @@ void nf_destroy(nf_plan *plan);
  */
 int nf_set_sink_slabs(nf_plan *plan, int x_first, int n_slabs);
 
+/*
+ * The other half of the slab decomposition (one process per GPU; the transfers themselves are the caller's point-to-point
+ * sends over NCCL / NVLink): everything that looks at particle data runs on the device, by the cell rule of nf_bin.
+ *
+ * nf_slab_histogram -- particles per x-slab of a position array.
+ *   pos_dev [n][3] device, hist_host [cpd] host (OVERWRITTEN).  Synchronises.  NF_ERR_DOMAIN as nf_bin.
+ * nf_slab_select -- stable compaction: the particles of pos_dev whose cell has x index in {x_first, ..., x_first +
+ *   n_slabs - 1} (mod cpd), in their original relative order (so that the receiver's stable cell sort reproduces the
+ *   order a whole-box plan sees inside every cell), copied device to device into
+ *   out_dev [cap][3]; idx_out_dev [cap] (or NULL) receives their input indices (for payloads that travel with the
+ *   particle, e.g. masses); *m_host = number selected.  NF_ERR_NOMEM if it exceeds cap.  Synchronises.
+ * nf_get_slab_cost -- cost_host [cpd] (OVERWRITTEN): pair interactions per x-slab of the last binning, sum over the slab's
+ *   cells of count x (particles in the cell's stencil) -- the scheduler's exact cost; 0 for slabs outside the sink slabs
+ *   (their cells are sources only on this rank: the owner reports them).  Ranks add their vectors (all-reduce) to get the
+ *   whole box.  Synchronises.  NF_ERR_STATE without a binning.
+ * nf_slab_partition -- HOST ONLY, no device, no plan: world contiguous slab ranges first[r], count[r] covering 0..cpd-1,
+ *   every rank at least one slab, minimising the largest range cost ("contiguous x-slabs balanced by
+ *   interaction cost"; "a contiguous span of slabs").  cost == NULL: equal costs.  NF_ERR_ARG unless
+ *   1 <= world <= cpd and every cost is finite and >= 0.
+ */
+int nf_slab_histogram(nf_plan *plan, const float *pos_dev, long long n, long long *hist_host);
+int nf_slab_select(nf_plan *plan, const float *pos_dev, long long n, int x_first, int n_slabs, float *out_dev,
+                   unsigned *idx_out_dev, long long cap, long long *m_host);
+int nf_get_slab_cost(nf_plan *plan, double *cost_host);
+int nf_slab_partition(const double *cost, int cpd, int world, int *first, int *count);
+
 /* ---- host-buffer entry points (end-to-end path: the copies are part of the call) ------------- */
 
 /* Copies pos_host [n][3] to a plan-owned device buffer (async if pinned) and runs nf_bin on it. */

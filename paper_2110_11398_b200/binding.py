@@ -24,6 +24,7 @@ EXPORTS = [
     "nf_plan_create", "nf_bin", "nf_rebin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_masses", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
+    "nf_slab_histogram", "nf_slab_select", "nf_get_slab_cost", "nf_slab_partition",
 ]
 
 
@@ -98,6 +99,14 @@ def _load() -> ctypes.CDLL:
     lib.nf_get_stats.argtypes = [vp, ctypes.POINTER(nf_stats)]
     lib.nf_set_option.restype = i32
     lib.nf_set_option.argtypes = [vp, ctypes.c_char_p, ll]
+    lib.nf_slab_histogram.restype = i32
+    lib.nf_slab_histogram.argtypes = [vp, vp, ll, ctypes.POINTER(ll)]
+    lib.nf_slab_select.restype = i32
+    lib.nf_slab_select.argtypes = [vp, vp, ll, i32, i32, vp, vp, ll, ctypes.POINTER(ll)]
+    lib.nf_get_slab_cost.restype = i32
+    lib.nf_get_slab_cost.argtypes = [vp, ctypes.POINTER(dbl)]
+    lib.nf_slab_partition.restype = i32
+    lib.nf_slab_partition.argtypes = [ctypes.POINTER(dbl), i32, i32, ctypes.POINTER(i32), ctypes.POINTER(i32)]
     return lib
 
 
@@ -249,6 +258,43 @@ def nf_set_option(plan: int, key: str, value: int) -> None:
     _check(_lib.nf_set_option(plan, key.encode(), int(value)))
 
 
+def nf_slab_histogram(plan: int, pos: torch.Tensor, cpd: int) -> list[int]:
+    pos = _dev_f32(pos, "pos")
+    h = (ctypes.c_longlong * cpd)()
+    _check(_lib.nf_slab_histogram(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0], h))
+    return list(h)
+
+
+def nf_slab_select(plan: int, pos: torch.Tensor, x_first: int, n_slabs: int, cap: int, want_index: bool = False):
+    """Returns (selected positions [m][3], input indices [m] int64 or None); ``cap`` = an upper bound of m."""
+    pos = _dev_f32(pos, "pos")
+    out = torch.empty((max(int(cap), 0), 3), dtype=torch.float32, device=pos.device)
+    idx = torch.empty((max(int(cap), 0),), dtype=torch.int32, device=pos.device) if want_index else None
+    m = ctypes.c_longlong(0)
+    _check(_lib.nf_slab_select(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0], int(x_first), int(n_slabs),
+                               ctypes.c_void_p(out.data_ptr()) if out.numel() else None,
+                               ctypes.c_void_p(idx.data_ptr()) if (idx is not None and idx.numel()) else None, out.shape[0], ctypes.byref(m)))
+    return out[:m.value], (idx[:m.value].to(torch.int64) if idx is not None else None)
+
+
+def nf_get_slab_cost(plan: int, cpd: int) -> list[float]:
+    c = (ctypes.c_double * cpd)()
+    _check(_lib.nf_get_slab_cost(plan, c))
+    return list(c)
+
+
+def nf_slab_partition(cost, cpd: int, world: int) -> list[tuple[int, int]]:
+    """Host-only: contiguous slab ranges (first, count) with balanced cost; ``cost`` None = equal costs."""
+    first, count = (ctypes.c_int * world)(), (ctypes.c_int * world)()
+    carr = None
+    if cost is not None:
+        if len(cost) != cpd:
+            raise ValueError("cost must have cpd entries")
+        carr = (ctypes.c_double * cpd)(*[float(v) for v in cost])
+    _check(_lib.nf_slab_partition(carr, int(cpd), int(world), first, count))
+    return [(first[r], count[r]) for r in range(world)]
+
+
 def nf_get_stats(plan: int) -> dict:
     st = nf_stats()
     _check(_lib.nf_get_stats(plan, ctypes.byref(st)))
@@ -377,6 +423,17 @@ class Plan:
         self._use_current_stream()
         nf_accel_host(self._h, out_host)
         return out_host
+
+    def slab_histogram(self, pos: torch.Tensor) -> list[int]:
+        self._use_current_stream()
+        return nf_slab_histogram(self._h, pos, self.cpd)
+
+    def slab_select(self, pos: torch.Tensor, x_first: int, n_slabs: int, cap: int, want_index: bool = False):
+        self._use_current_stream()
+        return nf_slab_select(self._h, pos, x_first, n_slabs, cap, want_index)
+
+    def slab_cost(self) -> list[float]:
+        return nf_get_slab_cost(self._h, self.cpd)
 
     def binning(self) -> dict:
         return nf_get_binning(self._h, self.n, self.ncells)

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnf_b200.so")
-SOURCES = ["nf_api.cu", "nf_bin.cu", "nf_direct.cu"]
+SOURCES = ["nf_api.cu", "nf_bin.cu", "nf_direct.cu", "nf_slabs.cu"]
 HEADERS = [os.path.join(CSRC, "nf_internal.h"), os.path.join(HERE, "..", "include", "nf.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -547,37 +547,52 @@ def test_kick_errors_and_empty():
 
 
 # ---------------------------------------------------------------- x-slab decomposition (NEXT 3), ranks emulated one after another
-@pytest.mark.parametrize("idx,n_side,cpd,world", [(3, 40, 10, 2), (4, 40, 10, 3), (1, 32, 9, 4), (2, 48, 5, 2)])
-def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, world):
-    """Each emulated rank bins its slabs plus the halo its peers would send (slabs.select_for_peer, the function
-    halo_exchange ships) and computes its own sinks: bit-identical to the whole-box plan, interaction counts add up."""
+@pytest.mark.parametrize("idx,n_side,cpd,world,balanced", [(3, 40, 10, 2, False), (4, 40, 10, 3, True), (1, 32, 9, 4, True),
+                                                           (2, 48, 5, 2, False), (4, 48, 12, 4, True), (5, 40, 10, 5, True)])
+def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, world, balanced):
+    """Each emulated rank bins its slabs plus the halo its peers would send (slabs.pack_for_peers: nf_slab_histogram +
+    nf_slab_select on the device, the function halo_exchange ships) and computes its own sinks: bit-identical to the
+    whole-box plan, interaction counts add up.  Ranges: equal slab counts, or balanced by the library's slab costs."""
     import paper_2110_11398_b200 as nf
     from paper_2110_11398_b200 import slabs
     cfg = nf_inputs.scaled(idx, n_side, cpd)
     pos = nf_inputs.generate(cfg)
+    pos_d = pos.cuda()
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
         plan.set_option("window", 64)       # any window: equal on every plan
-        plan.bin(pos.cuda())
+        plan.bin(pos_d)
         whole = plan.accel().cpu()
         total = plan.stats()["interactions"]
-    sl = slabs.slab_of(pos, cfg.cpd, cfg.L)
-    parts = slabs.slab_partition(cfg.cpd, world)
-    owned = [pos[((sl - f) % cfg.cpd) < c].contiguous() for f, c in parts]
-    idx_owned = [torch.nonzero(((sl - f) % cfg.cpd) < c).squeeze(1) for f, c in parts]
+        cost = plan.slab_cost()
+        assert sum(cost) == total                                      # the scheduler's exact cost, per slab
+        parts = slabs.slab_partition(cfg.cpd, world, cost if balanced else None)
+        sel = slabs.LibrarySelector(plan)
+        b = oracle_mod.bin_particles(pos.numpy(), cfg.cpd, cfg.L)
+        sl_ref = (b["cid"] // (cfg.cpd * cfg.cpd)).astype(np.int64)
+        assert sel.histogram(pos_d) == np.bincount(sl_ref, minlength=cfg.cpd).tolist()
+        owned, idx_owned = [], []
+        for f, c in parts:
+            o, i = plan.slab_select(pos_d, f, c, pos.shape[0], want_index=True)
+            ref_i = np.nonzero(((sl_ref - f) % cfg.cpd) < c)[0]
+            assert np.array_equal(i.cpu().numpy(), ref_i) and torch.equal(o.cpu(), pos[ref_i])      # stable, exact copies
+            owned.append(o.contiguous())
+            idx_owned.append(i.cpu())
+        sends = [slabs.pack_for_peers(owned[q], cfg.cpd, cfg.R, q, world, parts, sel)[0] for q in range(world)]
+    assert sum(c for _, c in parts) == cfg.cpd and all(c >= 1 for _, c in parts)
     got = torch.full_like(whole, float("nan"))
     inter = 0
     for r, (f, c) in enumerate(parts):
-        halos = [slabs.select_for_peer(owned[q], slabs.slab_of(owned[q], cfg.cpd, cfg.L), parts[r], cfg.cpd, cfg.R)
-                 for q in range(world) if q != r]
-        local = torch.cat([owned[r]] + halos).contiguous()
+        local = torch.cat([owned[r]] + [sends[q][r] for q in range(world) if q != r]).contiguous()
         with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
             plan.set_sink_slabs(f, c)
             plan.set_option("window", 64)
-            plan.bin(local.cuda())
+            plan.bin(local)
             acc = torch.full((local.shape[0], 3), 7.0, device="cuda")
             plan.accel(acc)
             torch.cuda.synchronize()
             inter += plan.stats()["interactions"]
+            mine = plan.slab_cost()                                     # owned slabs only: the ranks' vectors add up
+            assert all(mine[s] == (cost[s] if ((s - f) % cfg.cpd) < c else 0.0) for s in range(cfg.cpd))
         acc = acc.cpu()
         assert torch.all(acc[owned[r].shape[0]:] == 7.0)              # halo rows are not written
         got[idx_owned[r]] = acc[:owned[r].shape[0]]
@@ -585,6 +600,9 @@ def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, worl
     assert inter == total
     ref = oracle_mod.accel(pos.numpy(), cfg.cpd, cfg.L, cfg.eps, cfg.R)
     assert_parity(got.numpy().astype(np.float64), ref, f"{cfg.name} in {world} slab ranges")
+    if balanced:                                                       # the point of the cost partition: the slowest rank's share
+        load = lambda pp: max(sum(cost[(f + i) % cfg.cpd] for i in range(c)) for f, c in pp)
+        assert load(parts) <= load(slabs.slab_partition(cfg.cpd, world)) * (1 + 1e-12)
 
 
 def test_sink_slab_errors():

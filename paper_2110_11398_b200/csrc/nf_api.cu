@@ -37,7 +37,7 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     const size_t nonempty = N < C ? N : C;
     const size_t pmax = N + 3 * nonempty + 8;
     const size_t ncol = (size_t)cpd * cpd;
-    const size_t umax = (N < ncol ? N : ncol) + N / 32 + 2;    // every column ends with one ragged window; windows >= 32 sinks
+    const size_t umax = (N < ncol ? N : ncol) + N / 16 + 2;    // every column ends with one ragged window; the others hold >= 64 of the <= 4 N padded slots
     const size_t nsort = (N + 1 > umax ? N + 1 : umax);          // the unit order reuses the sort buffers
     int sort_passes = 1, sort_bits = kSortMinBits;
     sort_plan((unsigned long long)C, &sort_passes, &sort_bits);
@@ -467,7 +467,8 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
     }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
     if (!strcmp(key, "window") && v >= 0 && v % 32 == 0 && v <= kChunk) {
-        p->window = (int)v; p->binned = false; return NF_OK;
+        p->window = (int)((v + kGroup - 1) / kGroup * kGroup);     // whole sink groups of 64 slots
+        p->binned = false; return NF_OK;
     }
     set_error("unknown option or bad value: %s = %lld", key, v);
     return NF_ERR_ARG;

@@ -487,18 +487,19 @@ __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t 
     }
 }
 
-// work units per z-column: windows of kChunk consecutive cell-sorted sinks
-// Length of the next window of a column that has `rem` sinks left.  Whole windows of `chunk`; the remainder of a
-// column with default windows is cut so that its sink groups (32 sinks each) divide the consumer warps: 5-7 groups ->
-// 128 sinks (4 groups) first, 3 groups -> 64 sinks (2 groups) first.  Every window then keeps all the warps of its CTA
+// work units per z-column: windows of k.chunk consecutive PADDED slots (sink slots; a lane of the direct kernel holds an
+// aligned pair of them, and cells are padded to multiples of 4 slots, so a pair never straddles two cells).
+// Length of the next window of a column that has `rem` slots left.  Whole windows of `chunk`; the remainder of a
+// column with default windows is cut so that its sink groups (64 slots each) divide the consumer warps: 5-7 groups ->
+// 256 slots (4 groups) first, 3 groups -> 128 slots (2 groups) first.  Every window then keeps all the warps of its CTA
 // busy (the warps without sinks share the stages, nf_direct.cu); 3, 5, 6 or 7 groups would leave 2-3 of them idle.
 __device__ __forceinline__ uint32_t window_len(uint32_t rem, uint32_t chunk)
 {
     if (rem >= chunk) return chunk;
     if (chunk == (uint32_t)kChunk && kConsumerWarps == 8) {
-        const uint32_t ng = (rem + 31u) >> 5;
-        if (ng >= 5 && ng <= 7) return 128u;
-        if (ng == 3) return 64u;
+        const uint32_t ng = (rem + (uint32_t)kGroup - 1u) / (uint32_t)kGroup;
+        if (ng >= 5 && ng <= 7) return 4u * kGroup;
+        if (ng == 3) return 2u * kGroup;
     }
     return rem;
 }
@@ -509,24 +510,25 @@ __device__ __forceinline__ uint32_t windows_in(uint32_t ncol, uint32_t chunk)
     return nw;
 }
 
-__global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ offset,
+__global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ poff,
                                                        uint32_t *__restrict__ nunits)
 {
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
-    const uint32_t ncol = offset[(size_t)(col + 1) * k.cpd] - offset[(size_t)col * k.cpd];
+    const uint32_t ncol = poff[(size_t)(col + 1) * k.cpd] - poff[(size_t)col * k.cpd];
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
     nunits[col] = rel < k.nslab ? windows_in(ncol, (uint32_t)k.chunk) : 0u;      // columns outside the sink slabs: sources only
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
-__global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ offset,
+__global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ poff, const uint32_t *__restrict__ count,
                                                     const uint32_t *__restrict__ src, const uint32_t *__restrict__ ubase,
                                                     Unit *__restrict__ units, uint32_t *__restrict__ ukey)
 {
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
-    const uint32_t *off = offset + (size_t)col * k.cpd;
+    const uint32_t *off = poff + (size_t)col * k.cpd;
+    const uint32_t *cn = count + (size_t)col * k.cpd;
     const uint32_t *sc = src + (size_t)col * k.cpd;
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
     if (rel >= k.nslab) return;
@@ -538,12 +540,12 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
         const uint32_t s1 = s0 + len;
         while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
         Unit un;
-        un.s0 = s0; un.col = col; un.ns = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
-        unsigned long long cost = 0;
+        un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
+        unsigned long long cost = 0;                      // exact pair interactions of the window's real sinks
         int zz = z;
         for (;;) {
-            const uint32_t lo = max(off[zz], s0), hi = min(off[zz + 1], s1);
-            cost += (unsigned long long)(hi - lo) * sc[zz];
+            const uint32_t lo = max(off[zz], s0), hi = min(off[zz] + cn[zz], s1);
+            if (hi > lo) cost += (unsigned long long)(hi - lo) * sc[zz];
             if (off[zz + 1] >= s1) break;
             zz++;
         }
@@ -601,15 +603,16 @@ static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free
     const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
     uint32_t *ukey = (uint32_t *)ws.units_sorted;
     cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions);  L++;
-    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.offset, ws.ubase);  L++;
+    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.poff, ws.ubase);  L++;
     exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
-    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.offset, ws.src, ws.ubase, ws.units, ukey);  L++;
+    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.poff, ws.count, ws.src, ws.ubase, ws.units, ukey);  L++;
     NF_CUDA_OK(cudaGetLastError());
 
     // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
     const size_t ncol_sink = (size_t)k.nslab * k.cpd;
-    const size_t umax = (n < ncol_sink ? n : ncol_sink) + n / (size_t)(k.chunk < 32 ? 32 : k.chunk) + 2 * ncol_sink + 2;
-    const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 32 + 2;            // what carve() reserved
+    const size_t pmax = n + 3 * (n < (size_t)k.ncells ? n : (size_t)k.ncells);            // padded slots
+    const size_t umax = (n < ncol_sink ? n : ncol_sink) + pmax / (size_t)(k.chunk < kGroup ? kGroup : k.chunk) + 2 * ncol_sink + 2;
+    const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 16 + 2;            // what carve() reserved
     const size_t ub = umax < ucap ? umax : ucap;
     if (p->heavy_first) {
         const int rc = radix_pass(ukey, nullptr, free_key, free_val, ub, 0, kSortMinBits, true, false, false, g, ws.radix_hist,
@@ -624,18 +627,17 @@ static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free
 int launch_bin(nf_plan *p, const float *pos, long long n_ll)
 {
     const size_t n = (size_t)n_ll;
-    // sinks per work unit: the caller's window, else kChunk -- except for a problem so small that its units would not
-    // fill the grid of persistent CTAs: there the longest of 256, 128, 64 that still gives every CTA slot a unit (the
-    // consumer warps of a short window share its stages, nf_direct.cu).  Config 1 (32^3 particles): 567 units of 64
-    // sinks, 0.137 ms against 0.238 ms for 162 units of 256.
+    // sink slots per work unit: the caller's window, else kChunk -- except for a problem so small that its units would not
+    // fill the grid of persistent CTAs: there the longest of 512, 256, 128, 64 that still gives every CTA slot a unit (the
+    // consumer warps of a short window share its stages, nf_direct.cu).
     p->k.chunk = kChunk;
     if (p->window > 0) p->k.chunk = p->window;
     else if (n_ll > 0) {
         const double cols = (double)p->k.nslab * p->k.cpd;
-        const double per_col = (double)n_ll / ((double)p->k.cpd * p->k.cpd);
+        const double per_col = 1.03 * (double)n_ll / ((double)p->k.cpd * p->k.cpd);      // padded slots, roughly
         const double slots = (double)p->sm_count * kMinCtasPerSm;
         int w = kChunk;
-        while (w > 64 && cols * std::ceil(per_col / w) < slots) w >>= 1;    // 256, 128, 64: sink-group counts that divide the consumer warps
+        while (w > kGroup && cols * std::ceil(per_col / w) < slots) w >>= 1;    // sink-group counts that divide the consumer warps
         p->k.chunk = w;
     }
     const Consts &k = p->k;

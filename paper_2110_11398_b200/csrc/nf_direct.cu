@@ -5,9 +5,9 @@
 //   O(N^2) summation with a compact spline softening kernel"; periodic images kept).
 //
 // Design (sm_100a):
-//   * a work unit is a WINDOW of <= kChunk consecutive cell-sorted sinks of one z-column (cells are z-fastest,
-//     so a column is one contiguous run of the sorted order): every warp holds 32 real sinks whatever the
-//     cell occupancy -- no lane is lost to the ~68-particles-per-cell granularity;
+//   * a work unit is a WINDOW of <= kChunk consecutive PADDED sink slots of one z-column (cells are z-fastest,
+//     so a column is one contiguous run of the source arrays): every warp holds 64 slots whatever the cell
+//     occupancy -- only the pad slots (cells are padded to multiples of 4) are idle sinks;
 //   * persistent CTAs, one producer warp + kConsumerWarps consumer warps, units pulled from an atomic
 //     counter in heavy-first order;
 //   * for each of the (2R+1)^2 neighbour columns the producer streams the z-run of cells [z0-R, z1+R] that the
@@ -17,8 +17,11 @@
 //     pointer), so no lane ever evaluates a pair outside its stencil; the order pairs the lanes of a warp by
 //     source cell (step s takes the cell j with (j - z0 + R) mod (2R+1) == s), so lanes of neighbouring sink
 //     cells read the same piece except in the one step where their stencils do not overlap;
-//   * one sink per lane in registers; sources are read as LDS.128 of 4 x, 4 y, 4 z and processed as two
-//     packed pairs with FFMA2/FADD2/FMUL2 (fma.rn.f32x2), one MUFU.RSQ per interaction;
+//   * TWO sinks per lane in registers, an aligned pair of padded slots (always the same cell), packed as the two
+//     halves of f32x2 operands; sources are read as LDS.128 of 4 x, 4 y, 4 z and every source is a scalar
+//     broadcast against the sink pair: FADD2 / FFMA2 / FMUL2 (fma.rn.f32x2) do two interactions each, one
+//     MUFU.RSQ per interaction.  Every shared-memory load, every piece lookup and every loop instruction of a
+//     lane serves twice the interactions it would with one sink per lane;
 //   * coordinates are cell-corner relative (exact); the periodic wrap and the cell-to-cell shift are one
 //     constant per (sink cell, source cell) subtracted from the sink once per piece -- nothing periodic
 //     in the pair loop;
@@ -45,8 +48,8 @@ struct __align__(16) StageDesc {
     int      j0;               // cell of pieces[0], as an index relative to z0 - R
     int      soft_mode;        // 2: spline body everywhere; 1: for |oz| <= 1 (column with |ox|,|oy| <= 1); 0: never
     float    dx, dy;           // sink shift of this column: d = x_src - (x_sink - shift), scaled units
-    uint32_t s0;               // unit: first sorted slot
-    uint32_t ns;               //       sinks
+    uint32_t p0;               // unit: first padded sink slot
+    uint32_t np;               //       padded sink slots
     uint32_t z0, z1;           //       first / last sink cell (z index)
     uint32_t colbase;          //       col * cpd
     int      oxy;              // column offset: (ox + 128) | (oy + 128) << 8
@@ -65,7 +68,7 @@ struct __align__(128) SharedStorageT {
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
-    double part[kConsumerWarps][4][32];   // short windows: per-warp partial sums (x, y, z, rho) of a split unit
+    double part[kConsumerWarps][8][32];   // short windows: per-warp partial sums (x, y, z, rho of the lane's two sinks) of a split unit
 };
 
 // ---- PTX helpers: mbarrier + TMA 1-D bulk copy ---------------------------------------------------
@@ -111,72 +114,26 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 }
 
 // ---- pair bodies -------------------------------------------------------------------------------
+// A lane holds two sinks A, B; every float2 below is (value for A, value for B).  PACKED: f32x2 instructions (FADD2, FFMA2,
+// FMUL2: two interactions each; a source coordinate enters as a scalar broadcast operand); otherwise scalar FP32 (variant 1).
 constexpr float kSelfR2 = 2e-36f;   // r^2 of a pair at r = 0 is the offset `tiny` = 1e-36 (spline law); nothing else is below this
 struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin)
 
-// a += k d for two packed interactions.  A packed FFMA2 with three distinct register-pair operands holds the
-// register-file read ports 3 cycles for 2 cycles of pipe; NF_SCALAR_ACC of the three components (x, y, z order)
-// are issued as two scalar FFMA instead (2 cycles, one more issue slot each).
-#ifndef NF_SCALAR_ACC
-#define NF_SCALAR_ACC 0
-#endif
-template <int COMP>
-__device__ __forceinline__ void accum2(const float2 k, const float2 d, float2 &a)
+template <bool PACKED> __device__ __forceinline__ float2 add2(const float2 a, const float2 b)
 {
-    if (COMP < NF_SCALAR_ACC) { a.x = fmaf(k.x, d.x, a.x); a.y = fmaf(k.y, d.y, a.y); }
-    else a = __ffma2_rn(k, d, a);
+    return PACKED ? __fadd2_rn(a, b) : make_float2(a.x + b.x, a.y + b.y);
 }
-
-// two sources (packed) against one sink, Newtonian body: 11 FP32-pipe instructions per pair of interactions
-// (3 FADD2, 6 FFMA2, 2 FMUL2) plus 2 MUFU.RSQ; with source masses M one more FMUL2 (k m)
-template <bool MASS>
-__device__ __forceinline__ void interact2(const float2 X, const float2 Y, const float2 Z, const float2 M, const float2 nx, const float2 ny,
-                                          const float2 nz, const SoftCoef &c, float2 &ax, float2 &ay, float2 &az)
+template <bool PACKED> __device__ __forceinline__ float2 mul2(const float2 a, const float2 b)
 {
-    const float2 dx = __fadd2_rn(X, nx), dy = __fadd2_rn(Y, ny), dz = __fadd2_rn(Z, nz);
-    float2 r2 = __ffma2_rn(dz, dz, make_float2(c.tiny, c.tiny));
-    r2 = __ffma2_rn(dy, dy, r2);
-    r2 = __ffma2_rn(dx, dx, r2);
-    float2 ri;
-    ri.x = rsqrt_approx(r2.x);
-    ri.y = rsqrt_approx(r2.y);
-    const float2 ri2 = __fmul2_rn(ri, ri);
-    float2 k = __fmul2_rn(ri2, ri);
-    if (MASS) k = __fmul2_rn(k, M);
-    accum2<0>(k, dx, ax);
-    accum2<1>(k, dy, ay);
-    accum2<2>(k, dz, az);
+    return PACKED ? __fmul2_rn(a, b) : make_float2(a.x * b.x, a.y * b.y);
 }
-
-// scalar body (variant 1): 14 / 11 FP32-pipe instructions per interaction (+ 3 with the density estimate).
-// MODE 0: Newtonian, 1: spline, 2: spline + kernel density weight max(0, 1 - r^2/b^2)
-template <int MODE, bool MASS>
-__device__ __forceinline__ void interact1(const float X, const float Y, const float Z, const float M, const float nx, const float ny,
-                                          const float nz, const SoftCoef &c, float &ax, float &ay, float &az, float &rho)
+template <bool PACKED> __device__ __forceinline__ float2 fma2(const float2 a, const float2 b, const float2 c)
 {
-    const float dx = X + nx, dy = Y + ny, dz = Z + nz;
-    const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, c.tiny)));
-    const float ri = rsqrt_approx(r2);
-    float k = ri * ri * ri;
-    if (MODE >= 1) {
-        const float r = r2 * ri;
-        const float t = fmaf(fmaf(r, c.C, c.B), r, c.A);
-        k = fminf(k, t);
-        // with masses the capped k of the self pair (r^2 = tiny; the cap is 3e38 for eps = 0) times m could overflow to
-        // inf and inf * 0 = NaN: the self pair and exactly coincident particles are dropped explicitly (reading C5)
-        if (MASS && r2 <= kSelfR2) k = 0.f;
-    }
-    if (MODE == 2) {                      // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
-        const float q2 = c.plummer ? fmaf(dx, dx, fmaf(dy, dy, dz * dz)) : r2;
-        rho += fmaxf(fmaf(q2, c.nb2, 1.0f), 0.0f);
-    }
-    if (MASS) k *= M;
-    ax = fmaf(k, dx, ax);
-    ay = fmaf(k, dy, ay);
-    az = fmaf(k, dz, az);
+    return PACKED ? __ffma2_rn(a, b, c) : make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y));
 }
+__device__ __forceinline__ float2 bc(const float v) { return make_float2(v, v); }
 
-// FP32 partial sums of one (sink, stage): two chains per component (packed: the two halves of an f32x2)
+// FP32 partial sums of one (sink pair, stage)
 struct Partial {
     float2 x, y, z, rho;
     __device__ __forceinline__ void clear() { x = y = z = rho = make_float2(0.f, 0.f); }
@@ -186,86 +143,96 @@ constexpr uint32_t kFull = 0xffffffffu;
 #ifndef NF_UNROLL_SOFT
 #define NF_UNROLL_SOFT 2
 #endif
-constexpr int kUnrollSoft = NF_UNROLL_SOFT;
+constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable piece loop
 #ifndef NF_UNROLL_TAIL
-#define NF_UNROLL_TAIL 8
+#define NF_UNROLL_TAIL 4
 #endif
-constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)   // unrolling of the spline-capable piece loop
+constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
 
-// Newtonian part of two packed interactions: d, r^2, 1/r and k = r^-3
-__device__ __forceinline__ void pair_head(const float2 X, const float2 Y, const float2 Z, const float2 nx, const float2 ny,
-                                          const float2 nz, const float tiny, float2 &dx, float2 &dy, float2 &dz, float2 &r2,
-                                          float2 &ri, float2 &k)
+// Newtonian part of one source against the sink pair: d, r^2, 1/r and k = r^-3.  11 FP32-pipe lane-operations per
+// interaction (3 add, 6 fma, 2 mul) plus one MUFU.RSQ; n = shift - sink, so d = source + n.
+template <bool PACKED>
+__device__ __forceinline__ void src_head(const float xs, const float ys, const float zs, const float2 nx, const float2 ny, const float2 nz,
+                                         const float tiny, float2 &dx, float2 &dy, float2 &dz, float2 &r2, float2 &ri, float2 &k)
 {
-    dx = __fadd2_rn(X, nx); dy = __fadd2_rn(Y, ny); dz = __fadd2_rn(Z, nz);
-    r2 = __ffma2_rn(dz, dz, make_float2(tiny, tiny));
-    r2 = __ffma2_rn(dy, dy, r2);
-    r2 = __ffma2_rn(dx, dx, r2);
+    dx = add2<PACKED>(nx, bc(xs)); dy = add2<PACKED>(ny, bc(ys)); dz = add2<PACKED>(nz, bc(zs));
+    r2 = fma2<PACKED>(dz, dz, bc(tiny));
+    r2 = fma2<PACKED>(dy, dy, r2);
+    r2 = fma2<PACKED>(dx, dx, r2);
     ri.x = rsqrt_approx(r2.x);
     ri.y = rsqrt_approx(r2.y);
-    k = __fmul2_rn(__fmul2_rn(ri, ri), ri);
+    k = mul2<PACKED>(mul2<PACKED>(ri, ri), ri);
 }
-__device__ __forceinline__ void pair_spline(const float2 r2, const float2 ri, const SoftCoef &c, float2 &k)
+template <bool PACKED>
+__device__ __forceinline__ void src_spline(const float2 r2, const float2 ri, const SoftCoef &c, float2 &k)
 {
-    const float2 r = __fmul2_rn(r2, ri);                    // t = (C r + B) r + A: one register constant per FFMA2
-    float2 t = __ffma2_rn(r, make_float2(c.C, c.C), make_float2(c.B, c.B));
-    t = __ffma2_rn(t, r, make_float2(c.A, c.A));
+    const float2 r = mul2<PACKED>(r2, ri);                  // t = (C r + B) r + A
+    float2 t = fma2<PACKED>(r, bc(c.C), bc(c.B));
+    t = fma2<PACKED>(t, r, bc(c.A));
     k.x = fminf(k.x, t.x);
     k.y = fminf(k.y, t.y);
 }
-// kernel density weights of two packed interactions: rho += max(0, 1 - r^2/b^2)
-__device__ __forceinline__ void pair_density(const float2 r2, const SoftCoef &c, float2 &rho)
+// kernel density weights: rho += max(0, 1 - r^2/b^2)
+template <bool PACKED>
+__device__ __forceinline__ void src_density(const float2 r2, const SoftCoef &c, float2 &rho)
 {
-    float2 w = __ffma2_rn(r2, make_float2(c.nb2, c.nb2), make_float2(1.0f, 1.0f));
+    float2 w = fma2<PACKED>(r2, bc(c.nb2), bc(1.0f));
     w.x = fmaxf(w.x, 0.0f);
     w.y = fmaxf(w.y, 0.0f);
-    rho = __fadd2_rn(rho, w);
+    rho = add2<PACKED>(rho, w);
+}
+template <bool PACKED>
+__device__ __forceinline__ void src_accum(const float2 k, const float2 dx, const float2 dy, const float2 dz, Partial &f)
+{
+    f.x = fma2<PACKED>(k, dx, f.x); f.y = fma2<PACKED>(k, dy, f.y); f.z = fma2<PACKED>(k, dz, f.z);
 }
 
-// Four sources against the sink of every lane.  With MODE >= 1 exactly the lanes of `mask` must call it together
-// (warp vote inside): the spline is evaluated only when some lane of the warp has a pair of this quad inside eps_s -- a
-// fraction of a percent of the quads at production density; otherwise the body is the Newtonian one plus
-// three FMNMX, a vote and a branch.
+// Two sources against the sink pair of every lane (four interactions).  MODE 0: Newtonian.  MODE >= 1: exactly the lanes of
+// `mask` must call it together (warp vote inside): the spline is evaluated only when some lane of the warp has one of these
+// pairs inside eps_s -- a fraction of a percent of the calls at production density; otherwise the body is the Newtonian one
+// plus three FMNMX, a vote and a branch.  MODE 2 adds the kernel density weight the same way (sources within b).
 template <bool PACKED, int MODE, bool MASS>
-__device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float4 M, const float sxi, const float syi,
-                                     const float szi, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
+__device__ __forceinline__ void duo(const float xa, const float ya, const float za, const float ma, const float xb, const float yb,
+                                    const float zb, const float mb, const float2 nx, const float2 ny, const float2 nz,
+                                    const SoftCoef &c, Partial &f, const uint32_t mask)
 {
-    if (PACKED && MODE == 0) {
-        const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        interact2<MASS>(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), make_float2(M.x, M.y), nx, ny, nz, c, f.x, f.y, f.z);
-        interact2<MASS>(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), make_float2(M.z, M.w), nx, ny, nz, c, f.x, f.y, f.z);
-    } else if (PACKED) {
-        const float2 nx = make_float2(sxi, sxi), ny = make_float2(syi, syi), nz = make_float2(szi, szi);
-        float2 dxa, dya, dza, r2a, ria, ka, dxb, dyb, dzb, r2b, rib, kb;
-        pair_head(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y), nx, ny, nz, c.tiny, dxa, dya, dza, r2a, ria, ka);
-        pair_head(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w), nx, ny, nz, c.tiny, dxb, dyb, dzb, r2b, rib, kb);
+    float2 dxa, dya, dza, r2a, ria, ka, dxb, dyb, dzb, r2b, rib, kb;
+    src_head<PACKED>(xa, ya, za, nx, ny, nz, c.tiny, dxa, dya, dza, r2a, ria, ka);
+    src_head<PACKED>(xb, yb, zb, nx, ny, nz, c.tiny, dxb, dyb, dzb, r2b, rib, kb);
+    if (MODE >= 1) {
         const float m = fminf(fminf(r2a.x, r2a.y), fminf(r2b.x, r2b.y));
         if (__any_sync(mask, m < c.soft_r2)) {
-            pair_spline(r2a, ria, c, ka);
-            pair_spline(r2b, rib, c, kb);
-            if (MASS) {                       // see interact1: drop r = 0 before the mass multiplies the capped k
+            src_spline<PACKED>(r2a, ria, c, ka);
+            src_spline<PACKED>(r2b, rib, c, kb);
+            if (MASS) {
+                // with masses the capped k of the self pair (r^2 = tiny; the cap is 3e38 for eps = 0) times m could overflow to
+                // inf and inf * 0 = NaN: the self pair and exactly coincident particles are dropped explicitly (reading C5)
                 ka.x = r2a.x > kSelfR2 ? ka.x : 0.f; ka.y = r2a.y > kSelfR2 ? ka.y : 0.f;
                 kb.x = r2b.x > kSelfR2 ? kb.x : 0.f; kb.y = r2b.y > kSelfR2 ? kb.y : 0.f;
             }
         }
-        if (MODE == 2 && __any_sync(mask, m < c.dens_r2)) {     // some lane has a source of this quad inside b
+        if (MODE == 2 && __any_sync(mask, m < c.dens_r2)) {     // some lane has one of these sources inside b
             if (c.plummer) {                  // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
-                r2a = __ffma2_rn(dxa, dxa, __ffma2_rn(dya, dya, __fmul2_rn(dza, dza)));
-                r2b = __ffma2_rn(dxb, dxb, __ffma2_rn(dyb, dyb, __fmul2_rn(dzb, dzb)));
+                r2a = fma2<PACKED>(dxa, dxa, fma2<PACKED>(dya, dya, mul2<PACKED>(dza, dza)));
+                r2b = fma2<PACKED>(dxb, dxb, fma2<PACKED>(dyb, dyb, mul2<PACKED>(dzb, dzb)));
             }
-            pair_density(r2a, c, f.rho);
-            pair_density(r2b, c, f.rho);
+            src_density<PACKED>(r2a, c, f.rho);
+            src_density<PACKED>(r2b, c, f.rho);
         }
-        if (MASS) { ka = __fmul2_rn(ka, make_float2(M.x, M.y)); kb = __fmul2_rn(kb, make_float2(M.z, M.w)); }
-        accum2<0>(ka, dxa, f.x); accum2<1>(ka, dya, f.y); accum2<2>(ka, dza, f.z);
-        accum2<0>(kb, dxb, f.x); accum2<1>(kb, dyb, f.y); accum2<2>(kb, dzb, f.z);
-    } else {
-        interact1<MODE, MASS>(X.x, Y.x, Z.x, M.x, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
-        interact1<MODE, MASS>(X.y, Y.y, Z.y, M.y, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
-        interact1<MODE, MASS>(X.z, Y.z, Z.z, M.z, sxi, syi, szi, c, f.x.x, f.y.x, f.z.x, f.rho.x);
-        interact1<MODE, MASS>(X.w, Y.w, Z.w, M.w, sxi, syi, szi, c, f.x.y, f.y.y, f.z.y, f.rho.y);
     }
+    if (MASS) { ka = mul2<PACKED>(ka, bc(ma)); kb = mul2<PACKED>(kb, bc(mb)); }
+    src_accum<PACKED>(ka, dxa, dya, dza, f);
+    src_accum<PACKED>(kb, dxb, dyb, dzb, f);
+}
+
+// Four sources (one LDS.128 of x, y, z[, m]) against the sink pair of every lane: eight interactions.
+template <bool PACKED, int MODE, bool MASS>
+__device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float4 M, const float2 nx, const float2 ny,
+                                     const float2 nz, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
+{
+    duo<PACKED, MODE, MASS>(X.x, Y.x, Z.x, M.x, X.y, Y.y, Z.y, M.y, nx, ny, nz, c, f, mask);
+    duo<PACKED, MODE, MASS>(X.z, Y.z, Z.z, M.z, X.w, Y.w, Z.w, M.w, nx, ny, nz, c, f, mask);
 }
 
 // One step of a warp: every lane runs over ITS piece (n4 quads at px).  `live` = lanes that have a piece in this
@@ -275,7 +242,7 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 // converged for the vote of the spline body.
 template <bool PACKED, int MODE, bool MASS>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
-                                           const uint32_t live, const int jdummy, const float sxi, const float syi, const float szi,
+                                           const uint32_t live, const int jdummy, const float2 nx, const float2 ny, const float2 nz,
                                            const SoftCoef &c, Partial &f)
 {
     const float4 *__restrict__ py = px + kTileAlloc / 4;
@@ -285,20 +252,20 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
     if (n4 > 0) {
         if (MODE == 0) {
 #pragma unroll 2
-            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f);
         } else {
 #pragma unroll kUnrollSoft
-            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f, live);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f, live);
         }
     }
     __syncwarp();
 #pragma unroll kUnrollTail
     for (int j = nmin; j < nmax; j++) {
-        if (MODE >= 1 && PACKED) {                    // the body votes: keep the warp converged
+        if (MODE >= 1) {                              // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
-            quad<PACKED, MODE, MASS>(px[jj], py[jj], pz[jj], MASS ? pm[jj] : one, sxi, syi, szi, c, f);
+            quad<PACKED, MODE, MASS>(px[jj], py[jj], pz[jj], MASS ? pm[jj] : one, nx, ny, nz, c, f);
         } else if (j < n4) {
-            quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, sxi, syi, szi, c, f);
+            quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f);
         }
     }
 }
@@ -415,7 +382,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.p0 = un.p0; d.np = un.np; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -462,7 +429,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.s0 = un.s0; d.ns = un.ns; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.p0 = un.p0; d.np = un.np; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -500,47 +467,57 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;
-    float xi = 0.f, yi = 0.f, zi = 0.f;
-    double ax = 0.0, ay = 0.0, az = 0.0, oczs = 0.0, rho = 0.0;
-    // A window of fewer than kChunk sinks leaves consumer warps without sinks.  They take a share of the unit's stages
-    // instead: with ng = ceil(ns / 32) sink groups the kConsumerWarps / ng warps {g, g + ng, g + 2 ng, ...} hold the SAME
-    // 32 sinks, warp q of them computes the stages q, q + nsplit, ... of the unit, and the partial sums meet in shared
+    float2 xi = make_float2(0.f, 0.f), yi = xi, zi = xi;         // the lane's two sinks (A, B): an aligned pair of padded slots
+    double axA = 0.0, ayA = 0.0, azA = 0.0, axB = 0.0, ayB = 0.0, azB = 0.0, rhoA = 0.0, rhoB = 0.0, oczs = 0.0;
+    // A window of fewer than kChunk slots leaves consumer warps without sinks.  They take a share of the unit's stages
+    // instead: with ng = ceil(np / 64) sink groups the kConsumerWarps / ng warps {g, g + ng, g + 2 ng, ...} hold the SAME
+    // 64 slots, warp q of them computes the stages q, q + nsplit, ... of the unit, and the partial sums meet in shared
     // memory at the end of the unit, added in the fixed order q = 0, 1, ... (deterministic).  Small problems, whose units
     // cannot fill the machine, and the ragged last window of every column then keep all warps of the CTA busy.
     // one register: nsplit (warps sharing the sinks) | ng << 4 (sink groups) | q << 8 (this warp's share) | countdown << 12
     static_assert(kConsumerWarps <= 15, "the split state packs warp counts into 4-bit fields");
     uint32_t sp = 1u | ((uint32_t)kConsumerWarps << 4);
     int zrel = 0, zoff = 0;             // the lane's sink cell relative to z0, and zrel mod (2R+1)
-    uint32_t slot = 0;                  // the lane's sorted slot (perm index)
+    uint32_t slot = 0;                  // sorted slot (perm index) of sink A; sink B is slot + 1
     uint32_t cell = 0;                  // the lane's sink cell id
-    bool act = false, warp_on = false;
+    uint32_t nreal = 0;                 // how many of the lane's two slots hold a particle to write (0, 1, 2)
+    bool warp_on = false;
     for (;;) {
         mbar_wait(&sm.full[stage], phase);
         const StageDesc &d = sm.desc[stage];
         const int flags = d.flags;
         if (flags & kFlagTerm) break;
         if (flags & kFlagBegin) {
-            const uint32_t ns = d.ns;
-            const int ng = (int)((ns + 31u) >> 5), nsplit = kConsumerWarps / ng, q = warp / ng;
+            const uint32_t np = d.np;
+            const int ng = (int)((np + (uint32_t)kGroup - 1u) / (uint32_t)kGroup), nsplit = kConsumerWarps / ng, q = warp / ng;
             sp = (uint32_t)nsplit | ((uint32_t)ng << 4) | ((uint32_t)q << 8) | ((uint32_t)q << 12);   // first stage of warp q: stage q
-            const uint32_t kk = (uint32_t)((warp - q * ng) * 32 + lane);
+            const uint32_t kk = (uint32_t)((warp - q * ng) * kGroup + 2 * lane);
             warp_on = q < nsplit;
-            act = warp_on && kk < ns;
-            ax = ay = az = rho = 0.0;
+            const bool act = warp_on && kk < np;
+            axA = ayA = azA = axB = ayB = azB = rhoA = rhoB = 0.0;
+            nreal = 0;
             if (warp_on) {
-                // lanes past the end of a ragged window shadow its last sink (same pieces, nothing written)
-                slot = d.s0 + (act ? kk : ns - 1u);
-                const uint32_t *off = a.offset + d.colbase;
+                // lanes past the end of a ragged window shadow its last pair (same pieces, nothing written)
+                const uint32_t p = d.p0 + (act ? kk : np - 2u);
+                const uint32_t *pof = a.poff + d.colbase;
                 int lo = (int)d.z0, hi = (int)d.z1;
-                while (lo < hi) {                      // last cell of [z0, z1] whose first slot is <= slot
+                while (lo < hi) {                      // last cell of [z0, z1] whose first padded slot is <= p
                     const int mid = (lo + hi + 1) >> 1;
-                    if (__ldg(off + mid) <= slot) lo = mid; else hi = mid - 1;
+                    if (__ldg(pof + mid) <= p) lo = mid; else hi = mid - 1;
                 }
                 zrel = lo - (int)d.z0;
                 zoff = zrel % nsteps;
-                if (EPI) cell = d.colbase + (uint32_t)lo;
-                const uint32_t p = __ldg(a.poff + d.colbase + lo) + (slot - __ldg(off + lo));
-                xi = __ldg(a.x + p); yi = __ldg(a.y + p); zi = __ldg(a.z + p);
+                cell = d.colbase + (uint32_t)lo;
+                const uint32_t o0 = __ldg(a.offset + cell), o1 = __ldg(a.offset + cell + 1);
+                slot = o0 + (p - __ldg(pof + lo));
+                if (act) nreal = slot + 1u < o1 ? 2u : (slot < o1 ? 1u : 0u);
+                const float2 X2 = __ldg(reinterpret_cast<const float2 *>(a.x + p));      // p is even: 8-byte aligned
+                const float2 Y2 = __ldg(reinterpret_cast<const float2 *>(a.y + p));
+                const float2 Z2 = __ldg(reinterpret_cast<const float2 *>(a.z + p));
+                xi = X2; yi = Y2; zi = Z2;
+                // a pad slot next to a real sink takes the real sink's coordinates: it then computes the same (unwritten)
+                // sums and never widens the gap tests below (a pad sits at 2^55)
+                if (slot < o1 && slot + 1u >= o1) { xi.y = xi.x; yi.y = yi.x; zi.y = zi.x; }
                 oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
             }
         }
@@ -548,17 +525,17 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
         sp = mine ? (sp | (((sp & 15u) - 1u) << 12)) : sp - (1u << 12);
         if (mine) {
             const int np = d.npieces, soft_mode = d.soft_mode;
-            const float sxi = d.dx - xi, syi = d.dy - yi;           // -(x_i - shift)
+            const float2 nx = make_float2(d.dx - xi.x, d.dx - xi.y), ny = make_float2(d.dy - yi.x, d.dy - yi.y);   // shift - sink
             const int ibase = zrel - d.j0;
-            // squared gap between the sink and the neighbour column (0 for the own column): a cell whose
-            // nearest face is farther than eps_s cannot hold a pair that needs the spline
+            // squared gap between the sinks and the neighbour column (0 for the own column): a cell whose
+            // nearest face is farther than eps_s cannot hold a pair that needs the spline.  The smaller of the two sinks' gaps.
             float gxy2 = 0.f;
             const int ox = (d.oxy & 255) - 128, oy = (d.oxy >> 8) - 128;
             const bool near_col = ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1;
             const bool gap_dens = DENS && a.dens_mode == 1 && near_col;
             if (soft_mode == 1 || gap_dens) {
-                const float gx = ox < 0 ? xi : (ox > 0 ? a.k.w_scaled - xi : 0.f);
-                const float gy = oy < 0 ? yi : (oy > 0 ? a.k.w_scaled - yi : 0.f);
+                const float gx = ox < 0 ? fminf(xi.x, xi.y) : (ox > 0 ? a.k.w_scaled - fmaxf(xi.x, xi.y) : 0.f);
+                const float gy = oy < 0 ? fminf(yi.x, yi.y) : (oy > 0 ? a.k.w_scaled - fmaxf(yi.x, yi.y) : 0.f);
                 gxy2 = fmaf(gx, gx, gy * gy);
             }
             const float4 *sbase = reinterpret_cast<const float4 *>(&sm.buf[stage][0][0]);
@@ -583,56 +560,62 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 if (nmax == 0) continue;
                 const int nmin = __reduce_min_sync(kFull, n4 > 0 ? n4 : 0x7fffffff);   // over the lanes that have a piece
                 const uint32_t live = __ballot_sync(kFull, n4 > 0);
-                const float szi = (float)(czs - oczs) - zi;
+                const float dzc = (float)(czs - oczs);
+                const float2 nz = make_float2(dzc - zi.x, dzc - zi.y);
                 const float4 *px = sbase + (sm_off >> 2);
                 const int jdummy = (kTile - sm_off) >> 2;           // the dummy quad, relative to px
                 const int dt = t - R;
                 bool soft = soft_mode == 2, dens = DENS && a.dens_mode == 2;
                 if (soft_mode == 1 || gap_dens) {                   // warp-uniform; dt is per lane
                     const bool touching = n4 > 0 && dt >= -1 && dt <= 1;
-                    const float gz = dt < 0 ? zi : (dt > 0 ? a.k.w_scaled - zi : 0.f);
+                    const float gz = dt < 0 ? fminf(zi.x, zi.y) : (dt > 0 ? a.k.w_scaled - fmaxf(zi.x, zi.y) : 0.f);
                     const float gap2 = fmaf(gz, gz, gxy2);
                     if (soft_mode == 1) soft = __any_sync(kFull, touching && gap2 < a.k.soft_thr2);
                     if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
-                if (DENS && dens) piece_loop<PACKED, 2, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
-                else if (soft)    piece_loop<PACKED, 1, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
-                else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, sxi, syi, szi, coef, f);
+                if (DENS && dens) piece_loop<PACKED, 2, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                else if (soft)    piece_loop<PACKED, 1, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
             }
-            ax += (double)f.x.x + (double)f.x.y;
-            ay += (double)f.y.x + (double)f.y.y;
-            az += (double)f.z.x + (double)f.z.y;
-            if (DENS) rho += (double)f.rho.x + (double)f.rho.y;
+            axA += (double)f.x.x; ayA += (double)f.y.x; azA += (double)f.z.x;
+            axB += (double)f.x.y; ayB += (double)f.y.y; azB += (double)f.z.y;
+            if (DENS) { rhoA += (double)f.rho.x; rhoB += (double)f.rho.y; }
         }
         if ((flags & kFlagEnd) && (sp & 15u) > 1u) {          // warp-uniform, the same for every consumer warp of the CTA
             const int nsplit = (int)(sp & 15u), ng = (int)((sp >> 4) & 15u), q = (int)((sp >> 8) & 15u);
             if (warp_on && q > 0) {
-                sm.part[warp][0][lane] = ax; sm.part[warp][1][lane] = ay; sm.part[warp][2][lane] = az;
-                if (DENS) sm.part[warp][3][lane] = rho;
+                sm.part[warp][0][lane] = axA; sm.part[warp][1][lane] = ayA; sm.part[warp][2][lane] = azA;
+                sm.part[warp][3][lane] = axB; sm.part[warp][4][lane] = ayB; sm.part[warp][5][lane] = azB;
+                if (DENS) { sm.part[warp][6][lane] = rhoA; sm.part[warp][7][lane] = rhoB; }
             }
             asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");
             if (warp_on && q == 0) {
                 for (int t = 1; t < nsplit; t++) {
                     const int w2 = warp + t * ng;
-                    ax += sm.part[w2][0][lane]; ay += sm.part[w2][1][lane]; az += sm.part[w2][2][lane];
-                    if (DENS) rho += sm.part[w2][3][lane];
+                    axA += sm.part[w2][0][lane]; ayA += sm.part[w2][1][lane]; azA += sm.part[w2][2][lane];
+                    axB += sm.part[w2][3][lane]; ayB += sm.part[w2][4][lane]; azB += sm.part[w2][5][lane];
+                    if (DENS) { rhoA += sm.part[w2][6][lane]; rhoB += sm.part[w2][7][lane]; }
                 }
             }
             asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");   // the buffer is free for the next unit
         }
-        if ((flags & kFlagEnd) && act && ((sp >> 8) & 15u) == 0u) {
-            const size_t i = __ldg(a.perm + slot);
+        if ((flags & kFlagEnd) && nreal && ((sp >> 8) & 15u) == 0u) {
             const double s2 = a.k.out_scale;
-            const float fx = (float)(ax * s2), fy = (float)(ay * s2), fz = (float)(az * s2);
-            if (!EPI || a.acc) { a.acc[3 * i + 0] = fx; a.acc[3 * i + 1] = fy; a.acc[3 * i + 2] = fz; }
-            if (DENS) a.rho[i] = (float)rho;
-            if (EPI && a.vel) {                                   // kick: v += a dt (leapfrog)
-                a.vel[3 * i + 0] = fmaf(fx, a.dt, a.vel[3 * i + 0]);
-                a.vel[3 * i + 1] = fmaf(fy, a.dt, a.vel[3 * i + 1]);
-                a.vel[3 * i + 2] = fmaf(fz, a.dt, a.vel[3 * i + 2]);
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                if ((uint32_t)h >= nreal) break;
+                const size_t i = __ldg(a.perm + slot + h);
+                const float fx = (float)((h ? axB : axA) * s2), fy = (float)((h ? ayB : ayA) * s2), fz = (float)((h ? azB : azA) * s2);
+                if (!EPI || a.acc) { a.acc[3 * i + 0] = fx; a.acc[3 * i + 1] = fy; a.acc[3 * i + 2] = fz; }
+                if (DENS) a.rho[i] = (float)(h ? rhoB : rhoA);
+                if (EPI && a.vel) {                                   // kick: v += a dt (leapfrog)
+                    a.vel[3 * i + 0] = fmaf(fx, a.dt, a.vel[3 * i + 0]);
+                    a.vel[3 * i + 1] = fmaf(fy, a.dt, a.vel[3 * i + 1]);
+                    a.vel[3 * i + 2] = fmaf(fz, a.dt, a.vel[3 * i + 2]);
+                }
+                if (EPI && a.amax)                             // per-cell max |a| of the timestep criterion
+                    atomicMax(a.amax + cell, __float_as_uint(sqrtf(fmaf(fx, fx, fmaf(fy, fy, fz * fz)))));
             }
-            if (EPI && a.amax)                             // per-cell max |a| of the timestep criterion
-                atomicMax(a.amax + cell, __float_as_uint(sqrtf(fmaf(fx, fx, fmaf(fy, fy, fz * fz)))));
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[stage]);

@@ -25,10 +25,11 @@ constexpr int kMaxR          = 127;               // the column offset travels a
 #define NF_STAGES_MASS 3
 #endif
 #ifndef NF_MIN_CTAS
-#define NF_MIN_CTAS 3
+#define NF_MIN_CTAS 2
 #endif
-constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // sink lanes per CTA = 32 * kConsumerWarps
-constexpr int kChunk         = 32 * kConsumerWarps;   // max sinks per work unit (a window of one z-column)
+constexpr int kConsumerWarps = NF_CONSUMER_WARPS; // consumer warps per CTA
+constexpr int kGroup         = 64;                // sink slots per warp: every lane holds TWO sinks (an aligned pair of padded slots)
+constexpr int kChunk         = kGroup * kConsumerWarps;   // max sink slots per work unit (a window of one z-column): 512
 constexpr int kTile          = NF_TILE;           // source slots per pipeline stage (multiple of 4)
 constexpr int kStages        = NF_STAGES;         // TMA pipeline depth (three staged arrays)
 constexpr int kStagesMass    = NF_STAGES_MASS;    //   with the fourth array of the mass kernels
@@ -60,11 +61,12 @@ inline void sort_plan(unsigned long long nkeys, int *passes, int *digit_bits)
     *passes = np; *digit_bits = b;
 }
 
-struct Unit {            // one work unit: a window of <= kChunk consecutive cell-sorted sinks of one z-column
-    uint32_t s0;         // first sorted slot (index into perm)
+struct Unit {            // one work unit: a window of <= kChunk consecutive PADDED slots of one z-column (the cells are padded
+                         // to multiples of 4 slots, so an aligned pair of slots never straddles two cells; pad slots are idle sinks)
+    uint32_t p0;         // first padded slot (index into the source arrays x, y, z), a multiple of 4
     uint32_t col;        // column id cx * cpd + cy
-    uint16_t ns;         // sinks in the window
-    uint16_t z0, z1;     // first and last cell (z index) that hold a sink of the window
+    uint16_t np;         // padded slots in the window, a multiple of 4
+    uint16_t z0, z1;     // first and last cell (z index) that hold a slot of the window
     uint16_t pad_;
 };
 
@@ -92,7 +94,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
 
 struct Consts {          // everything the kernels need about the problem, by value
     int cpd, R;
-    int chunk;                      // sinks per work unit (window of one z-column), 32..kChunk
+    int chunk;                      // sink slots per work unit (window of one z-column), 64..kChunk
     int slab0, nslab;               // sink slabs: cells with x index in {slab0, ..., slab0 + nslab - 1} mod cpd (default: all)
     uint32_t ncells;
     double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L

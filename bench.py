@@ -25,9 +25,27 @@ METRIC = "near_field_pair_interactions_per_s"
 UNIT = "interactions/s"
 FLOPS_PER_INTERACTION = 25      # 3 add + 8 fma(2) + 3 mul + 1 min + rsqrt(2): SURVEY.md 8(a) S6; the paper counts 26
 FLOPS_EXECUTED_MIN = 19         # the Newtonian body (3 add + 6 fma + 2 mul + rsqrt) the kernel runs where no pair is inside eps_s
-# DRAM bytes of one direct_kernel launch, ncu --set full (profiles/r1_v9_final_config3.md, profiles/r1_v8_final.md)
-NCU_TRAFFIC_BYTES = {"config3_uniform_256": 958413568 + 656910848, "config4_halos_512": 18155223000 + 5468523000}
 L2_BYTES = 126 * 1024 * 1024
+# ncu numbers are never measured by this run: they are READ from the committed capture summaries (one row per workload:
+# workload, dram bytes read, dram bytes written per direct_kernel launch, FMA-pipe busy %, issue-slot %, file of origin)
+NCU_TABLE = os.path.join(ROOT, "profiles", "r2_direct_kernel_counters.csv")
+
+
+def ncu_counters(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum (and the pipe counters) of one direct_kernel launch from the committed
+    `ncu --set full` capture of this workload, or None when no capture of it is committed."""
+    try:
+        import csv
+        with open(NCU_TABLE) as f:
+            for row in csv.DictReader(l for l in f if not l.startswith("#")):
+                if row["workload"] == workload:
+                    return {"traffic": int(float(row["dram_bytes_read"])) + int(float(row["dram_bytes_write"])),
+                            "fma_pipe_busy_pct": float(row["sm__pipe_fma_cycles_active_pct"]),
+                            "issue_active_pct": float(row["smsp__issue_active_pct"]),
+                            "source": "profiles/" + row["source"]}
+    except (OSError, KeyError, ValueError):
+        pass
+    return None
 
 
 def parse_args():
@@ -316,6 +334,32 @@ def run_config(idx, args, device_index, dist=None, with_e2e=True, steps=None, wa
             plan.set_masses(None)
             del mass
         if with_e2e:
+            # nf_rebin (the same particles after a drift of 0.004 cell widths rms, ~1 % of them change
+            # cell) beside the full nf_bin, for the generated (random) input order and for a caller that keeps its arrays in
+            # the library's cell order (pos[perm]); restores the timed binning afterwards
+            g = torch.Generator(device="cuda").manual_seed(4242)
+            cell = cfg.L / cfg.cpd
+            q = pos.clone()
+            rb = {}
+            for label in ("input_order_as_generated", "input_in_cell_order"):
+                plan.bin(q)
+                plan.bin(q)
+                full_ms = plan.stats()["ms_bin"]
+                t, movers, paths = [], [], []
+                for _ in range(3):
+                    q = torch.remainder(q + torch.randn(q.shape, generator=g, device="cuda") * (0.004 * cell), cfg.L)
+                    q[q >= cfg.L] = 0
+                    q = q.contiguous()
+                    torch.cuda.synchronize()
+                    plan.rebin(q)
+                    sr = plan.stats()
+                    t.append(sr["ms_bin"]); movers.append(sr["rebin_movers"]); paths.append(sr["rebin_path"])
+                rb[label] = {"ms_nf_bin": full_ms, "ms_nf_rebin": statistics.median(t), "speedup": full_ms / statistics.median(t),
+                             "movers_frac": statistics.median(movers) / cfg.n, "path": paths}
+                q = q[plan.binning()["perm"].long()].contiguous()
+            out["rebin"] = rb
+            del q
+            plan.bin(pos)
             pos_h = torch.empty(pos.shape, dtype=pos.dtype, pin_memory=True)
             pos_h.copy_(pos)
             acc_h = torch.empty(pos.shape, dtype=pos.dtype, pin_memory=True)
@@ -386,16 +430,19 @@ def main_b200(args):
         "ms_bin": s["ms_bin"], "ms_accel": s["ms_accel"],
         "e2e": {"value": world * I * r["e2e_steps"] / (e2e_ms / 1e3), "unit": UNIT, "h2d_bytes_per_step": 12 * n,
                 "d2h_bytes_per_step": 12 * n, "steps": r["e2e_steps"], "ms_per_step": e2e_ms / r["e2e_steps"],
-                "api": "nf_bin_host + nf_accel_host (pinned host buffers)"},
+                "api": "nf_bin_host + nf_accel_host (pinned host buffers)",
+                "frac_of_device_value": (world * I * r["e2e_steps"] / (e2e_ms / 1e3)) / value},
         "gpu_launches": K * (st["kernel_launches_bin"] + st["kernel_launches_accel"]),
         "clocks": r["clocks"],
         "roofline": {"bound": "alu", "kernel": "nf::direct_kernel<packed f32x2>", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg.name),
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": (ncu_counters(cfg.name) or {}).get("traffic"),
+                     "ncu": ncu_counters(cfg.name),
                      "executed": {"flops_per_interaction": FLOPS_EXECUTED_MIN,
                                   "achieved": achieved * FLOPS_EXECUTED_MIN / FLOPS_PER_INTERACTION,
                                   "frac": achieved * FLOPS_EXECUTED_MIN / FLOPS_PER_INTERACTION / peak,
                                   "note": "lower bound: quads with a pair inside eps_s execute the 25-flop body"},
-                     "attainable_frac": 0.88,
+                     "body_in_isolation": "the pair body alone (LDS.128 + the packed arithmetic, no scheduling) reaches 0.87 of this peak "
+                                          "at the kernel's 4 consumer warps per sub-partition: profiles/r2_ubench_fp32_pipe.md",
                      "peak_source": "SM count x 128 FP32 lanes x 2 x max SM clock read from the device (DESIGN.md)",
                      "sm_count": st["sm_count"], "clock_khz": st["clock_khz"], "launch_ms": ta * 1e3,
                      "grid": st["accel_grid"], "block": st["accel_block"]},
@@ -410,6 +457,8 @@ def main_b200(args):
         line["fused_kick"] = {"call": "nf_accel_kick: v += a dt and per-cell max |a| in the epilogue (PAPER.md:353, 212)",
                               "ms_accel": r["kick_ms_accel"], "overhead_frac": r["kick_ms_accel"] / (ta * 1e3) - 1.0,
                               "max_accel": r["amax_global"]}
+    if "rebin" in r:
+        line["rebin"] = dict(r["rebin"], call="nf_rebin after a drift of 0.004 cell widths rms (PAPER.md:353, 502; SURVEY 8(f) NEXT 4)")
     if "mass_ms_accel" in r:
         line["masses"] = {"call": "nf_set_masses (log-normal masses, sigma_ln 1) + nf_accel",
                           "ms_set_masses": r["mass_ms_set"], "ms_accel": r["mass_ms_accel"],

@@ -51,7 +51,9 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     ws.valA = (uint32_t *)take(4 * nsort);
     ws.valB = (uint32_t *)take(4 * nsort);
     ws.radix_hist = (uint32_t *)take(4 * hist_items);
-    ws.count  = (uint32_t *)take(4 * (C + 1));
+    ws.count  = (uint32_t *)take(4 * (C + 1));                  // count, interactions, scalars: zeroed by ONE memset (nf_bin.cu)
+    ws.interactions = (unsigned long long *)take(8 * 4);
+    ws.scalars      = (uint32_t *)take(4 * 64);
     ws.offset = (uint32_t *)take(4 * (C + 2));
     ws.poff   = (uint32_t *)take(4 * (C + 2));
     ws.ubase  = (uint32_t *)take(4 * (C + 2));
@@ -63,8 +65,6 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     ws.units        = (Unit *)take(sizeof(Unit) * umax);
     ws.units_sorted = (Unit *)take(sizeof(Unit) * umax);
     ws.bucket_hist  = (uint32_t *)take(4 * 256);
-    ws.interactions = (unsigned long long *)take(8 * 4);
-    ws.scalars      = (uint32_t *)take(4 * 64);
     ws.offset_new = (uint32_t *)take(4 * (C + 2));
     ws.arr_count  = (uint32_t *)take(4 * (C + 2));
     ws.arr_off    = (uint32_t *)take(4 * (C + 2));

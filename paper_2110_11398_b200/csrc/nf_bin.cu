@@ -106,10 +106,9 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const uint32_t *in, u
 constexpr int kSmallThreads = 1024, kSmallItems = 16, kSmallMax = kSmallThreads * kSmallItems;
 
 template <class Op>
-__global__ void __launch_bounds__(kSmallThreads) scan_small(const uint32_t *in, uint32_t *out, uint32_t n, Op op, int write_total,
-                                                            uint32_t *total_out)
+__device__ __forceinline__ void scan_small_body(const uint32_t *in, uint32_t *out, uint32_t n, Op op, int write_total,
+                                                uint32_t *total_out, uint32_t *sm /*[33]*/)
 {
-    __shared__ uint32_t sm[33];
     const uint32_t base = threadIdx.x * kSmallItems;
     uint32_t v[kSmallItems], s = 0;
 #pragma unroll
@@ -123,6 +122,27 @@ __global__ void __launch_bounds__(kSmallThreads) scan_small(const uint32_t *in, 
         if (write_total) out[n] = tot;
         if (total_out) *total_out = tot;
     }
+}
+
+template <class Op>
+__global__ void __launch_bounds__(kSmallThreads) scan_small(const uint32_t *in, uint32_t *out, uint32_t n, Op op, int write_total,
+                                                            uint32_t *total_out)
+{
+    __shared__ uint32_t sm[33];
+    scan_small_body(in, out, n, op, write_total, total_out, sm);
+}
+
+// Small problems are bound by the number of launches of nf_bin: the three prefix sums that follow the cell-id kernel
+// (cell offsets, padded offsets, the digit histogram of the single sort pass) in one launch.
+__global__ void __launch_bounds__(kSmallThreads) small_scans_kernel(const uint32_t *count, uint32_t *offset, uint32_t *poff, uint32_t ncells,
+                                                                    uint32_t *hist, uint32_t nhist, uint32_t *padded_total)
+{
+    __shared__ uint32_t sm[33];
+    scan_small_body(count, offset, ncells, OpId(), 1, nullptr, sm);
+    __syncthreads();
+    scan_small_body(count, poff, ncells, OpPad4(), 1, padded_total, sm);
+    __syncthreads();
+    scan_small_body(hist, hist, nhist, OpId(), 0, nullptr, sm);
 }
 
 template <class Op>
@@ -427,7 +447,8 @@ static cudaError_t scatter_dispatch(bool iota, bool last, const uint32_t *kin, c
 // `last` (particle sort only) fuses the gather of `g` into the scatter.
 static int radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, uint32_t *vout, size_t n, int shift, int bits,
                       bool iota, bool last, bool have_hist, const GatherArgs &g, uint32_t *hist, uint32_t *scan_tmp,
-                      cudaStream_t st, int *launches, const uint32_t *n_dev = nullptr)   // n_dev: n is an upper bound, the count is on the device
+                      cudaStream_t st, int *launches, const uint32_t *n_dev = nullptr,   // n_dev: n is an upper bound, the count is on the device
+                      bool hist_scanned = false)
 {
     const uint32_t nb = (uint32_t)((n + kSortTile - 1) / kSortTile);
     const uint32_t bins = 1u << bits;
@@ -435,7 +456,7 @@ static int radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, 
         radix_hist_kernel<<<nb, kSortThreads, 0, st>>>(kin, n, shift, bins - 1u, hist, nb, n_dev);
         *launches += 1;
     }
-    exclusive_scan(hist, hist, (size_t)bins * nb, scan_tmp, OpId(), 0, nullptr, st, launches);
+    if (!hist_scanned) exclusive_scan(hist, hist, (size_t)bins * nb, scan_tmp, OpId(), 0, nullptr, st, launches);
     cudaError_t e;
     switch (bits) {
     case 8:  e = scatter_dispatch<8>(iota, last, kin, vin, kout, vout, n, shift, hist, nb, g, st, n_dev); break;
@@ -586,6 +607,118 @@ int launch_set_masses(nf_plan *p, const float *mass)
     return NF_OK;
 }
 
+// S5 of a small problem in ONE launch (one block): stencil counts and the exact interaction count, the units of every
+// column, heavy-first order by a counting sort on the cost key (not stable: the order of equal keys only matters for L2
+// locality, which a problem of this size has anyway; no result depends on the unit order).
+constexpr int kSmallCells = 2048, kSmallUnits = 4096;
+__global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint32_t *__restrict__ count, const uint32_t *__restrict__ poff,
+                                                           uint32_t *__restrict__ src_out, unsigned long long *__restrict__ interactions,
+                                                           Unit *__restrict__ units, Unit *__restrict__ units_sorted,
+                                                           uint32_t *__restrict__ scalars, int heavy_first)
+{
+    __shared__ uint32_t s_cnt[kSmallCells], s_src[kSmallCells], s_off[kSmallCells + 1], s_col[kSmallCells / 2 + 2], s_hist[66], s_cur[66];
+    __shared__ unsigned char s_key[kSmallUnits];
+    __shared__ unsigned long long s_inter;
+    const int cpd = k.cpd, R = k.R;
+    const uint32_t C = k.ncells, ncols = (uint32_t)cpd * cpd;
+    for (uint32_t c = threadIdx.x; c < C; c += 1024) s_cnt[c] = count[c];
+    for (uint32_t c = threadIdx.x; c <= C; c += 1024) s_off[c] = poff[c];
+    if (threadIdx.x < 66) { s_hist[threadIdx.x] = 0; s_cur[threadIdx.x] = 0; }
+    if (threadIdx.x == 0) s_inter = 0;
+    __syncthreads();
+    unsigned long long mine = 0;
+    for (uint32_t c = threadIdx.x; c < C; c += 1024) {
+        const int cz = c % cpd, cy = (c / cpd) % cpd, cx = c / (cpd * cpd);
+        uint32_t src = 0;
+        for (int ox = -R; ox <= R; ox++) {
+            int sx = cx + ox; sx += sx < 0 ? cpd : 0; sx -= sx >= cpd ? cpd : 0;
+            for (int oy = -R; oy <= R; oy++) {
+                int sy = cy + oy; sy += sy < 0 ? cpd : 0; sy -= sy >= cpd ? cpd : 0;
+                const uint32_t row = ((uint32_t)sx * cpd + sy) * cpd;
+                for (int oz = -R; oz <= R; oz++) {
+                    int sz = cz + oz; sz += sz < 0 ? cpd : 0; sz -= sz >= cpd ? cpd : 0;
+                    src += s_cnt[row + sz];
+                }
+            }
+        }
+        s_src[c] = src;
+        src_out[c] = src;
+        int rel = cx - k.slab0; rel += rel < 0 ? cpd : 0;
+        if (rel < k.nslab) mine += (unsigned long long)s_cnt[c] * src;      // sinks of the owned slabs only
+    }
+    if (mine) atomicAdd(&s_inter, mine);
+    __syncthreads();
+    for (uint32_t col = threadIdx.x; col < ncols; col += 1024) {
+        const uint32_t ncol = s_off[(col + 1) * cpd] - s_off[col * cpd];
+        int rel = (int)(col / (uint32_t)cpd) - k.slab0; rel += rel < 0 ? cpd : 0;
+        s_col[col] = rel < k.nslab ? windows_in(ncol, (uint32_t)k.chunk) : 0u;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {                             // exclusive scan of the units per column by one warp
+        uint32_t carry = 0;
+        for (uint32_t c0 = 0; c0 < ncols; c0 += 32) {
+            const uint32_t col = c0 + threadIdx.x;
+            const uint32_t v = col < ncols ? s_col[col] : 0u;
+            uint32_t inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if ((int)threadIdx.x >= o) inc += t; }
+            if (col < ncols) s_col[col] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (threadIdx.x == 0) { s_col[ncols] = carry; scalars[2] = carry; *interactions = s_inter; }
+    }
+    __syncthreads();
+    const uint32_t nu = s_col[ncols];
+    for (uint32_t col = threadIdx.x; col < ncols; col += 1024) {
+        if (s_col[col + 1] == s_col[col]) continue;
+        const uint32_t *off = s_off + (size_t)col * cpd;
+        const uint32_t *cn = s_cnt + (size_t)col * cpd, *sc = s_src + (size_t)col * cpd;
+        const uint32_t c_begin = off[0], c_end = off[cpd];
+        uint32_t u = s_col[col];
+        int z = 0;
+        for (uint32_t s0 = c_begin, len = 0; s0 < c_end; s0 += len, u++) {
+            len = window_len(c_end - s0, (uint32_t)k.chunk);
+            const uint32_t s1 = s0 + len;
+            while (off[z + 1] <= s0) z++;
+            Unit un;
+            un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
+            unsigned long long cost = 0;
+            int zz = z;
+            for (;;) {
+                const uint32_t lo = max(off[zz], s0), hi = min(off[zz] + cn[zz], s1);
+                if (hi > lo) cost += (unsigned long long)(hi - lo) * sc[zz];
+                if (off[zz + 1] >= s1) break;
+                zz++;
+            }
+            un.z1 = (uint16_t)zz;
+            units[u] = un;
+            const uint32_t key = (uint32_t)__clzll((long long)cost);
+            s_key[u] = (unsigned char)key;
+            atomicAdd(&s_hist[key], 1u);
+            z = zz;
+        }
+    }
+    if (!heavy_first) return;
+    __syncthreads();
+    if (threadIdx.x < 32) {                             // exclusive scan of the 66 key counts
+        uint32_t carry = 0;
+        for (int c0 = 0; c0 < 66; c0 += 32) {
+            const int q = c0 + (int)threadIdx.x;
+            const uint32_t v = q < 66 ? s_hist[q] : 0u;
+            uint32_t inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if ((int)threadIdx.x >= o) inc += t; }
+            if (q < 66) s_hist[q] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    __syncthreads();
+    for (uint32_t u = threadIdx.x; u < nu; u += 1024) {
+        const uint32_t key = s_key[u];
+        units_sorted[s_hist[key] + atomicAdd(&s_cur[key], 1u)] = units[u];       // each thread re-reads the units it may not have written:
+    }                                                                           // the __syncthreads above orders the global writes of the block
+}
+
 // ---- S5 on the stream: per-cell stencil counts + exact interaction count, units per column, units, heavy-first order.
 // free_key / free_val: two n-sized scratch arrays for the unit sort.
 static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free_val, int *Lp)
@@ -649,9 +782,8 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     if (n == 0) { p->launches_bin = 0; p->perm = ws.valA; return NF_OK; }
 
     NF_CUDA_OK(cudaEventRecord(p->ev[0], st));
-    NF_CUDA_OK(cudaMemsetAsync(ws.count, 0, 4 * (size_t)(k.ncells + 1), st));
-    NF_CUDA_OK(cudaMemsetAsync(ws.scalars, 0, 4 * 64, st));
-    NF_CUDA_OK(cudaMemsetAsync(ws.interactions, 0, 8, st));
+    // count, interactions and scalars are carved next to each other: one memset
+    NF_CUDA_OK(cudaMemsetAsync(ws.count, 0, (size_t)((char *)(ws.scalars + 64) - (char *)ws.count), st));
 
     // stable sort by cell id: the first pass's digit histogram comes out of the cell-id kernel, the last pass writes
     // perm and the padded SoA arrays (no sorted keys are stored)
@@ -660,9 +792,18 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     const uint32_t nbs = (uint32_t)((n + kSortTile - 1) / kSortTile);
     cellid_kernel<<<nbs, kSortThreads, 0, st>>>(pos, n, k, ws.cid, ws.count, ws.scalars, (1u << dbits) - 1u, ws.radix_hist, nbs);  L++;
 
+    // A small problem is bound by the NUMBER of launches (config 1: 0.137 ms for ~20 of them, as long as its nf_accel):
+    // one launch for the three prefix sums, one for the whole of S5 -- five stream operations in all.
+    const size_t pmax_small = n + 3 * (n < (size_t)k.ncells ? n : (size_t)k.ncells);
+    const bool small = passes == 1 && k.ncells <= (uint32_t)kSmallCells && ((size_t)nbs << dbits) <= (size_t)kSmallMax &&
+                       pmax_small / kGroup + 3 * (size_t)k.cpd * k.cpd + 2 <= (size_t)kSmallUnits;
     // prefix sums: offset (exported), padded offsets, unit bases
-    exclusive_scan(ws.count, ws.offset, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
-    exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
+    if (small) {
+        small_scans_kernel<<<1, kSmallThreads, 0, st>>>(ws.count, ws.offset, ws.poff, k.ncells, ws.radix_hist, nbs << dbits, &ws.scalars[3]);  L++;
+    } else {
+        exclusive_scan(ws.count, ws.offset, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
+        exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
+    }
 
     GatherArgs g;
     g.pos = pos; g.offset = ws.offset; g.poff = ws.poff; g.X = ws.x; g.Y = ws.y; g.Z = ws.z; g.k = k;
@@ -670,7 +811,7 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     uint32_t *kbuf[2] = {ws.keyA, ws.keyB}, *vbuf[2] = {ws.valA, ws.valB};
     for (int ps = 0; ps < passes; ps++) {
         const int rc = radix_pass(kin, vin, kbuf[ps & 1], vbuf[ps & 1], n, dbits * ps, dbits, ps == 0, ps == passes - 1, ps == 0, g,
-                                  ws.radix_hist, ws.scan_tmp, st, &L);
+                                  ws.radix_hist, ws.scan_tmp, st, &L, nullptr, small);
         if (rc != NF_OK) return rc;
         kin = kbuf[ps & 1]; vin = vbuf[ps & 1];
     }
@@ -679,7 +820,13 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     p->slotcell = nullptr;                                     // materialised by the first nf_rebin
     uint32_t *free_key = kbuf[passes & 1], *free_val = vbuf[passes & 1];   // the pair not holding the result
 
-    { const int rc = launch_units(p, n, free_key, free_val, &L); if (rc != NF_OK) return rc; }
+    if (small) {
+        small_units_kernel<<<1, 1024, 0, st>>>(k, ws.count, ws.poff, ws.src, ws.interactions, ws.units, ws.units_sorted, ws.scalars,
+                                               p->heavy_first);  L++;
+    } else {
+        const int rc = launch_units(p, n, free_key, free_val, &L);
+        if (rc != NF_OK) return rc;
+    }
     NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
     NF_CUDA_OK(cudaGetLastError());
     // domain flag + unit count: the one documented synchronisation of nf_bin, at the END of the call -- nothing is

@@ -145,7 +145,7 @@ constexpr uint32_t kFull = 0xffffffffu;
 #endif
 constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable piece loop
 #ifndef NF_UNROLL_TAIL
-#define NF_UNROLL_TAIL 4
+#define NF_UNROLL_TAIL 8
 #endif
 constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece

@@ -62,11 +62,16 @@ def parse_args():
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
                     help="N > 1: 'replicas' (the contract: one GPU per problem, no sharding) or 'slabs' (ONE box split "
                          "into x-slab ranges with an R-slab halo exchange inside every step: strong scaling)")
+    ap.add_argument("--occupancy-sweep", default=None, metavar="CPD[,CPD...]",
+                    help="instead of a config: 200^3 uniform particles binned into CPD^3 cells for every CPD of the list "
+                         "(default list with an empty string: 49,63,79,100,126,159 = 68 ... 2 particles per cell), nf_accel only: "
+                         "the void regime of the direct kernel (PAPER.md:512)")
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--fastpath", type=int, default=None)
     ap.add_argument("--heavy-first", type=int, default=None)
     ap.add_argument("--ctas-per-sm", type=int, default=None)
-    ap.add_argument("--window", type=int, default=None, help="sinks per work unit (nf_set_option window)")
+    ap.add_argument("--window", type=int, default=None, help="sink slots per work unit (nf_set_option window)")
+    ap.add_argument("--flat-below", type=int, default=None, help="nf_set_option flat_below (0: never take the flat loop)")
     return ap.parse_args()
 
 
@@ -175,7 +180,7 @@ def fp32_peak_tflops(stats):
 
 def apply_options(plan, args):
     for key, val in (("variant", args.variant), ("fastpath", args.fastpath), ("heavy_first", args.heavy_first),
-                     ("ctas_per_sm", args.ctas_per_sm), ("window", args.window)):
+                     ("ctas_per_sm", args.ctas_per_sm), ("window", args.window), ("flat_below", args.flat_below)):
         if val is not None:
             plan.set_option(key, val)
 
@@ -565,6 +570,38 @@ def main_slabs(args):
         dist.destroy_process_group()
 
 
+def main_occupancy_sweep(args):
+    """Particles per cell against the fraction of the FP32 peak: the paper's late-time loss is "many sparse (void) kernels"
+    (PAPER.md:512).  One JSON line; nf_accel only (3 timed launches per grid after one warm-up)."""
+    import torch
+    import paper_2110_11398_b200 as nf
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    cpds = [int(t) for t in args.occupancy_sweep.split(",") if t] or [49, 63, 79, 100, 126, 159]
+    n_side = 200
+    g = torch.Generator(device="cuda").manual_seed(5)
+    pos = torch.rand((n_side ** 3, 3), generator=g, device="cuda", dtype=torch.float32)
+    rows = []
+    for cpd in cpds:
+        with nf.Plan(cpd, 1.0, 1.0 / (40 * n_side), 2) as plan:
+            apply_options(plan, args)
+            plan.bin(pos)
+            acc = plan.accel()
+            torch.cuda.synchronize()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            ev[0].record()
+            for _ in range(3):
+                plan.accel(acc)
+            ev[1].record()
+            torch.cuda.synchronize()
+            ms = ev[0].elapsed_time(ev[1]) / 3
+            st = plan.stats()
+            rows.append({"cpd": cpd, "particles_per_cell": pos.shape[0] / cpd ** 3, "ms_accel": ms, "ms_bin": st["ms_bin"],
+                         "interactions_per_s": st["interactions"] / ms * 1e3,
+                         "fp32_peak_frac_25flop": FLOPS_PER_INTERACTION * st["interactions"] / (ms * 1e-3) / 1e12 / fp32_peak_tflops(st)})
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "workload": f"uniform {n_side}^3 particles, CPD varied", "dtype": "f32",
+                      "data": "synthetic", "sweep": rows}))
+
+
 def main_reference(args):
     """The reference arm of this tier is the oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -597,7 +634,9 @@ def main_reference(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.impl == "reference":
+    if a.occupancy_sweep is not None:
+        main_occupancy_sweep(a)
+    elif a.impl == "reference":
         main_reference(a)
     elif a.decomp == "slabs":
         main_slabs(a)

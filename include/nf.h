@@ -174,7 +174,7 @@ void nf_destroy(nf_plan *plan);
  * particles whose cell has x index in {x_first, ..., x_first + n_slabs - 1} (mod cpd) are SINKS; every binned
  * particle is still a source.  A rank bins its own slabs plus the R halo slabs of each x-neighbour and gets
  * exactly the accelerations a whole-box plan would give its particles (bit for bit when both plans use the same
- * "window" option; the automatic window of small problems depends on the number of owned columns); rows of acc that belong to particles
+ * "window" and "quad_vote" options; the automatic window of small problems depends on the number of owned columns); rows of acc that belong to particles
  * outside the sink slabs are not written, and nf_stats.interactions counts the owned sinks only.
  * Takes effect at the next nf_bin (it invalidates the current binning).  Default: all slabs.
  * Errors: NF_ERR_ARG unless 0 <= x_first < cpd and 1 <= n_slabs <= cpd.
@@ -257,12 +257,22 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
- *   "window"       sinks per work unit: a multiple of 32 up to 256, or 0 (default) = 256, except for problems whose
- *                  units would not fill the grid of persistent CTAs, which get the longest of 256, 128 and 64 that does.
+ *   "window"       sink slots (padded: cells are padded to multiples of 4) per work unit: a multiple of 32 up to 512, rounded
+ *                  up to whole sink groups of 64, or 0 (default) = 512, except for problems whose units would not fill the
+ *                  grid of persistent CTAs, which get the longest of 512, 256, 128 and 64 that does.
  *                  The warps of a CTA that a short window leaves without sinks share the unit's stages.
  *                  Shorter windows give a small problem more work units, but every unit streams its whole stencil
- *                  again.  With 256-sink windows the remainder of a column is cut into 128 / 64 / fewer sinks (sink
- *                  groups that divide the consumer warps).  Accelerations are bit-identical between plans only for equal windows.  Takes effect at the next nf_bin.
+ *                  again.  With 512-slot windows the remainder of a column is cut into 256 / 128 / fewer slots (sink
+ *                  groups that divide the consumer warps).  Accelerations are bit-identical between plans only for equal
+ *                  windows.  Takes effect at the next nf_bin.
+ *   "flat_below"   windows with fewer padded slots per spanned cell than this walk a lane's stencil run in one flat loop
+ *                  (sparse cells: DESIGN.md 7); default 14, 0 = never.  Takes effect at the next nf_bin.
+ *   "quad_vote"    -1 (default) = the direct-kernel instance that votes once per four sources in the spline-capable loop is
+ *                  launched when the fullest cell of the binning holds more than 4096 particles (the halo cells of clustered
+ *                  inputs spend nearly all their pairs in that loop); 0 = never, 1 = always.  The two instances agree to one ulp of the
+ *                  pairs that sit within 0.1 % of eps_s (the spline's min is taken wherever the vote fired): bit-identical
+ *                  results between plans (slab ranks against the whole box) or between nf_accel and the fused
+ *                  nf_accel_density pass (which always votes per two sources) need the same explicit setting.
  *   "softening"    0 = the compact spline of the method (default); 1 = Plummer softening, force
  *                  d (r^2 + eps^2)^(-3/2) with eps the plan's length: the law the paper compares against
  *                  ("converges only quadratically to the correct large-scale force law")

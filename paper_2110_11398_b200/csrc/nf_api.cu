@@ -210,7 +210,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     memset(p, 0, sizeof(*p));
     Consts &k = p->k;
     k.cpd = cpd; k.R = R; k.ncells = (uint32_t)cpd * cpd * cpd;
-    k.slab0 = 0; k.nslab = cpd; k.chunk = kChunk;
+    k.slab0 = 0; k.nslab = cpd; k.chunk = kChunk; k.flat_below = kFlatBelow;
     k.L = L; k.cell_w = L / cpd; k.inv_cell_w = (double)cpd / L;
     int e2 = 0;
     (void)std::frexp(k.cell_w, &e2);              // cell_w = m 2^e2, m in [0.5, 1)
@@ -221,7 +221,7 @@ nf_plan *nf_plan_create(int cpd, double L, double eps, int R)
     p->device = -1;
     p->stream = 0;
     p->ws_n = -1;
-    p->variant = 0; p->fastpath = 1; p->heavy_first = 1; p->ctas_per_sm = 0; p->window = 0;
+    p->variant = 0; p->fastpath = 1; p->heavy_first = 1; p->ctas_per_sm = 0; p->window = 0; p->quad_vote_opt = -1;
     g_err[0] = 0;
     return p;
 }
@@ -466,6 +466,8 @@ int nf_set_option(nf_plan *p, const char *key, long long v)
         return set_softening(p, (int)v);
     }
     if (!strcmp(key, "ctas_per_sm") && v >= 0 && v <= 32) { p->ctas_per_sm = (int)v; return NF_OK; }
+    if (!strcmp(key, "quad_vote") && v >= -1 && v <= 1) { p->quad_vote_opt = (int)v; return NF_OK; }
+    if (!strcmp(key, "flat_below") && v >= 0 && v <= 1024) { p->k.flat_below = (int)v; p->binned = false; return NF_OK; }
     if (!strcmp(key, "window") && v >= 0 && v % 32 == 0 && v <= kChunk) {
         p->window = (int)((v + kGroup - 1) / kGroup * kGroup);     // whole sink groups of 64 slots
         p->binned = false; return NF_OK;

@@ -473,11 +473,14 @@ static int radix_pass(const uint32_t *kin, const uint32_t *vin, uint32_t *kout, 
 // src[c] = particles in the (2R+1)^3 periodic stencil of cell c; interactions = sum_c count[c] * src[c].
 __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t *__restrict__ count,
                                                        uint32_t *__restrict__ src_out,
-                                                       unsigned long long *__restrict__ interactions)
+                                                       unsigned long long *__restrict__ interactions, uint32_t *__restrict__ max_count)
 {
     __shared__ unsigned long long red[8];
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long mine = 0;
+    uint32_t cmax = c < k.ncells ? count[c] : 0u;
+    cmax = __reduce_max_sync(0xffffffffu, cmax);
+    if ((threadIdx.x & 31) == 0 && cmax) atomicMax(max_count, cmax);
     if (c < k.ncells) {
         const int cpd = k.cpd, R = k.R;
         const int cz = c % cpd, cy = (c / cpd) % cpd, cx = c / (cpd * cpd);
@@ -517,10 +520,10 @@ __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t 
 __device__ __forceinline__ uint32_t window_len(uint32_t rem, uint32_t chunk)
 {
     if (rem >= chunk) return chunk;
-    if (chunk == (uint32_t)kChunk && kConsumerWarps == 8) {
+    if (chunk == (uint32_t)kChunk && (kConsumerWarps & (kConsumerWarps - 1)) == 0) {
+        // the largest power of two of groups below a group count that is not one itself: 3 -> 2, 5..7 -> 4, 9..15 -> 8
         const uint32_t ng = (rem + (uint32_t)kGroup - 1u) / (uint32_t)kGroup;
-        if (ng >= 5 && ng <= 7) return 4u * kGroup;
-        if (ng == 3) return 2u * kGroup;
+        if (ng & (ng - 1u)) return (1u << (31 - __clz(ng))) * (uint32_t)kGroup;
     }
     return rem;
 }
@@ -561,7 +564,7 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
         const uint32_t s1 = s0 + len;
         while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
         Unit un;
-        un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
+        un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
         unsigned long long cost = 0;                      // exact pair interactions of the window's real sinks
         int zz = z;
         for (;;) {
@@ -571,6 +574,7 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
             zz++;
         }
         un.z1 = (uint16_t)zz;
+        un.flat = (uint16_t)((uint32_t)un.np < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
         units[u] = un;
         ukey[u] = (uint32_t)__clzll((long long)cost);     // heavier -> smaller key
         z = zz;
@@ -621,7 +625,10 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
     __shared__ unsigned long long s_inter;
     const int cpd = k.cpd, R = k.R;
     const uint32_t C = k.ncells, ncols = (uint32_t)cpd * cpd;
-    for (uint32_t c = threadIdx.x; c < C; c += 1024) s_cnt[c] = count[c];
+    uint32_t cmax = 0;
+    for (uint32_t c = threadIdx.x; c < C; c += 1024) { s_cnt[c] = count[c]; cmax = max(cmax, s_cnt[c]); }
+    cmax = __reduce_max_sync(0xffffffffu, cmax);
+    if ((threadIdx.x & 31) == 0 && cmax) atomicMax(&scalars[7], cmax);
     for (uint32_t c = threadIdx.x; c <= C; c += 1024) s_off[c] = poff[c];
     if (threadIdx.x < 66) { s_hist[threadIdx.x] = 0; s_cur[threadIdx.x] = 0; }
     if (threadIdx.x == 0) s_inter = 0;
@@ -681,7 +688,7 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
             const uint32_t s1 = s0 + len;
             while (off[z + 1] <= s0) z++;
             Unit un;
-            un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.pad_ = 0;
+            un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
             unsigned long long cost = 0;
             int zz = z;
             for (;;) {
@@ -691,6 +698,7 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
                 zz++;
             }
             un.z1 = (uint16_t)zz;
+            un.flat = (uint16_t)((uint32_t)un.np < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
             units[u] = un;
             const uint32_t key = (uint32_t)__clzll((long long)cost);
             s_key[u] = (unsigned char)key;
@@ -735,7 +743,7 @@ static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free
     const unsigned nbc = (k.ncells + 255) / 256;
     const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
     uint32_t *ukey = (uint32_t *)ws.units_sorted;
-    cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions);  L++;
+    cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions, &ws.scalars[7]);  L++;
     colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.poff, ws.ubase);  L++;
     exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
     units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.poff, ws.count, ws.src, ws.ubase, ws.units, ukey);  L++;
@@ -831,11 +839,12 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     NF_CUDA_OK(cudaGetLastError());
     // domain flag + unit count: the one documented synchronisation of nf_bin, at the END of the call -- nothing is
     // enqueued after it, so the binning is complete on return whatever stream the caller uses next
-    uint32_t sc[4];
+    uint32_t sc[8];
     NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));
     NF_CUDA_OK(cudaStreamSynchronize(st));
     if (sc[0]) { set_error("nf_bin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
     p->n_units = (long long)sc[2];
+    p->max_count = sc[7];
     p->have_bin_time = true;
     p->launches_bin = L;
     return NF_OK;
@@ -1200,6 +1209,7 @@ int launch_rebin(nf_plan *p, const float *pos)
     }
     p->rebin_path = 1;
     p->n_units = (long long)sc[2];
+    p->max_count = sc[7];
     p->have_bin_time = true;
     p->launches_bin = L;
     return NF_OK;

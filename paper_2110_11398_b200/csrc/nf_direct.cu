@@ -32,6 +32,8 @@
 //   * the epilogue writes acc[perm[s]] directly (S7 fused, no sorted acceleration buffer).
 #include "nf_internal.h"
 
+#include <type_traits>
+
 namespace nf {
 
 enum { kFlagBegin = 1, kFlagEnd = 2, kFlagTerm = 4 };
@@ -53,6 +55,7 @@ struct __align__(16) StageDesc {
     uint32_t z0, z1;           //       first / last sink cell (z index)
     uint32_t colbase;          //       col * cpd
     int      oxy;              // column offset: (ox + 128) | (oy + 128) << 8
+    int      flat;             // unit flag: sparse window, flat loop
     Piece    pieces[kMaxPieces];
 };
 
@@ -68,7 +71,9 @@ struct __align__(128) SharedStorageT {
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
-    double part[kConsumerWarps][8][32];   // short windows: per-warp partial sums (x, y, z, rho of the lane's two sinks) of a split unit
+    double quadz[kStages][kTile / 4 + 1];   // flat loop: z corner (scaled, with box wrap) of the cell of every quad of the stage
+    double acc[kConsumerWarps][8][32];    // FP64 sums of every warp's sinks (x, y, z of sink A, x, y, z of sink B, rho A, rho B): kept here, not in
+                                          // 16 registers per lane; the warps of a split unit add theirs up from here at the end of the unit
 };
 
 // ---- PTX helpers: mbarrier + TMA 1-D bulk copy ---------------------------------------------------
@@ -149,6 +154,10 @@ constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable
 #endif
 constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
+#ifndef NF_FLUSH_QUADS
+#define NF_FLUSH_QUADS 6
+#endif
+constexpr int kFlushQuads = NF_FLUSH_QUADS;    // a step of at least this many quads ends its FP32 chain (24 sources per sink)
 
 // Newtonian part of one source against the sink pair: d, r^2, 1/r and k = r^-3.  11 FP32-pipe lane-operations per
 // interaction (3 add, 6 fma, 2 mul) plus one MUFU.RSQ; n = shift - sink, so d = source + n.
@@ -227,12 +236,49 @@ __device__ __forceinline__ void duo(const float xa, const float ya, const float 
 }
 
 // Four sources (one LDS.128 of x, y, z[, m]) against the sink pair of every lane: eight interactions.
-template <bool PACKED, int MODE, bool MASS>
+template <bool PACKED, int MODE, bool MASS, bool QV = false>
 __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float4 M, const float2 nx, const float2 ny,
                                      const float2 nz, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
 {
-    duo<PACKED, MODE, MASS>(X.x, Y.x, Z.x, M.x, X.y, Y.y, Z.y, M.y, nx, ny, nz, c, f, mask);
-    duo<PACKED, MODE, MASS>(X.z, Y.z, Z.z, M.z, X.w, Y.w, Z.w, M.w, nx, ny, nz, c, f, mask);
+    if (MODE != 1 || !QV) {
+        duo<PACKED, MODE, MASS>(X.x, Y.x, Z.x, M.x, X.y, Y.y, Z.y, M.y, nx, ny, nz, c, f, mask);
+        duo<PACKED, MODE, MASS>(X.z, Y.z, Z.z, M.z, X.w, Y.w, Z.w, M.w, nx, ny, nz, c, f, mask);
+        return;
+    }
+    // QV (the kernel instance launched when the binning holds heavy cells, nf_api: the halo cells of the clustered configs
+    // spend nearly all their interactions in this loop): ONE vote per quad.  The common path keeps d and k of the four
+    // sources; the rare branch forms r^2 and 1/r again (the same bits: same inputs, same instructions).  Config 4 +2.9 %,
+    // config 3 -1.2 % (16 bytes of spills at the 96-register budget) -- hence a separate instance, not the default.
+    const float xs[4] = {X.x, X.y, X.z, X.w}, ys[4] = {Y.x, Y.y, Y.z, Y.w}, zs[4] = {Z.x, Z.y, Z.z, Z.w}, ms[4] = {M.x, M.y, M.z, M.w};
+    float2 dx[4], dy[4], dz[4], k[4];
+    float m = 3.0e38f;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        float2 r2, ri;
+        src_head<PACKED>(xs[j], ys[j], zs[j], nx, ny, nz, c.tiny, dx[j], dy[j], dz[j], r2, ri, k[j]);
+        m = fminf(m, fminf(r2.x, r2.y));
+    }
+    if (__any_sync(mask, m < c.soft_r2)) {
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            float2 r2 = fma2<PACKED>(dz[j], dz[j], bc(c.tiny));
+            r2 = fma2<PACKED>(dy[j], dy[j], r2);
+            r2 = fma2<PACKED>(dx[j], dx[j], r2);
+            float2 ri;
+            ri.x = rsqrt_approx(r2.x);
+            ri.y = rsqrt_approx(r2.y);
+            src_spline<PACKED>(r2, ri, c, k[j]);
+            if (MASS) {                        // see duo: drop r = 0 before the mass multiplies the capped k
+                k[j].x = r2.x > kSelfR2 ? k[j].x : 0.f;
+                k[j].y = r2.y > kSelfR2 ? k[j].y : 0.f;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        if (MASS) k[j] = mul2<PACKED>(k[j], bc(ms[j]));
+        src_accum<PACKED>(k[j], dx[j], dy[j], dz[j], f);
+    }
 }
 
 // One step of a warp: every lane runs over ITS piece (n4 quads at px).  `live` = lanes that have a piece in this
@@ -240,7 +286,7 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 // in the ragged tail a lane that has run out of sources is predicated off (Newtonian body) or reads the stage's
 // dummy quad (coordinates 2^55: contributes exactly 0 to the force and to the density) so that the warp stays
 // converged for the vote of the spline body.
-template <bool PACKED, int MODE, bool MASS>
+template <bool PACKED, int MODE, bool MASS, bool QV = false>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
                                            const uint32_t live, const int jdummy, const float2 nx, const float2 ny, const float2 nz,
                                            const SoftCoef &c, Partial &f)
@@ -255,7 +301,7 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
             for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f);
         } else {
 #pragma unroll kUnrollSoft
-            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f, live);
+            for (int j = 0; j < nmin; j++) quad<PACKED, MODE, MASS, QV>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f, live);
         }
     }
     __syncwarp();
@@ -263,7 +309,7 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
     for (int j = nmin; j < nmax; j++) {
         if (MODE >= 1) {                              // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
-            quad<PACKED, MODE, MASS>(px[jj], py[jj], pz[jj], MASS ? pm[jj] : one, nx, ny, nz, c, f);
+            quad<PACKED, MODE, MASS, QV>(px[jj], py[jj], pz[jj], MASS ? pm[jj] : one, nx, ny, nz, c, f);
         } else if (j < n4) {
             quad<PACKED, MODE, MASS>(px[j], py[j], pz[j], MASS ? pm[j] : one, nx, ny, nz, c, f);
         }
@@ -382,7 +428,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.p0 = un.p0; d.np = un.np; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.p0 = un.p0; d.np = un.np; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -429,7 +475,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.p0 = un.p0; d.np = un.np; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.p0 = un.p0; d.np = un.np; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -458,7 +504,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI, bool MASS>
+template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS ? 4 : 3> &sm, const int warp, const int lane)
 {
     const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f,
@@ -468,15 +514,16 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
     int stage = 0;
     uint32_t phase = 0;
     float2 xi = make_float2(0.f, 0.f), yi = xi, zi = xi;         // the lane's two sinks (A, B): an aligned pair of padded slots
-    double axA = 0.0, ayA = 0.0, azA = 0.0, axB = 0.0, ayB = 0.0, azB = 0.0, rhoA = 0.0, rhoB = 0.0, oczs = 0.0;
+    double oczs = 0.0;
+    double (*acc64)[32] = sm.acc[warp];                          // [8][32]: this warp's FP64 sums, one column per lane
     // A window of fewer than kChunk slots leaves consumer warps without sinks.  They take a share of the unit's stages
     // instead: with ng = ceil(np / 64) sink groups the kConsumerWarps / ng warps {g, g + ng, g + 2 ng, ...} hold the SAME
     // 64 slots, warp q of them computes the stages q, q + nsplit, ... of the unit, and the partial sums meet in shared
     // memory at the end of the unit, added in the fixed order q = 0, 1, ... (deterministic).  Small problems, whose units
     // cannot fill the machine, and the ragged last window of every column then keep all warps of the CTA busy.
-    // one register: nsplit (warps sharing the sinks) | ng << 4 (sink groups) | q << 8 (this warp's share) | countdown << 12
-    static_assert(kConsumerWarps <= 15, "the split state packs warp counts into 4-bit fields");
-    uint32_t sp = 1u | ((uint32_t)kConsumerWarps << 4);
+    // one register: nsplit (warps sharing the sinks) | ng << 8 (sink groups) | q << 16 (this warp's share) | countdown << 24
+    static_assert(kConsumerWarps <= 255, "the split state packs warp counts into 8-bit fields");
+    uint32_t sp = 1u | ((uint32_t)kConsumerWarps << 8);
     int zrel = 0, zoff = 0;             // the lane's sink cell relative to z0, and zrel mod (2R+1)
     uint32_t slot = 0;                  // sorted slot (perm index) of sink A; sink B is slot + 1
     uint32_t cell = 0;                  // the lane's sink cell id
@@ -490,11 +537,12 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
         if (flags & kFlagBegin) {
             const uint32_t np = d.np;
             const int ng = (int)((np + (uint32_t)kGroup - 1u) / (uint32_t)kGroup), nsplit = kConsumerWarps / ng, q = warp / ng;
-            sp = (uint32_t)nsplit | ((uint32_t)ng << 4) | ((uint32_t)q << 8) | ((uint32_t)q << 12);   // first stage of warp q: stage q
+            sp = (uint32_t)nsplit | ((uint32_t)ng << 8) | ((uint32_t)q << 16) | ((uint32_t)q << 24);   // first stage of warp q: stage q
             const uint32_t kk = (uint32_t)((warp - q * ng) * kGroup + 2 * lane);
             warp_on = q < nsplit;
             const bool act = warp_on && kk < np;
-            axA = ayA = azA = axB = ayB = azB = rhoA = rhoB = 0.0;
+#pragma unroll
+            for (int c = 0; c < (DENS ? 8 : 6); c++) acc64[c][lane] = 0.0;
             nreal = 0;
             if (warp_on) {
                 // lanes past the end of a ragged window shadow its last pair (same pieces, nothing written)
@@ -521,8 +569,8 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
             }
         }
-        const bool mine = warp_on && (sp >> 12) == 0u;                  // countdown to this warp's next stage
-        sp = mine ? (sp | (((sp & 15u) - 1u) << 12)) : sp - (1u << 12);
+        const bool mine = warp_on && (sp >> 24) == 0u;                  // countdown to this warp's next stage
+        sp = mine ? (sp | (((sp & 255u) - 1u) << 24)) : sp - (1u << 24);
         if (mine) {
             const int np = d.npieces, soft_mode = d.soft_mode;
             const float2 nx = make_float2(d.dx - xi.x, d.dx - xi.y), ny = make_float2(d.dy - yi.x, d.dy - yi.y);   // shift - sink
@@ -541,6 +589,53 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
             const float4 *sbase = reinterpret_cast<const float4 *>(&sm.buf[stage][0][0]);
             Partial f;
             f.clear();
+            bool pending = true;
+            auto flush = [&]() {                                        // FP32 chain -> FP64 sums (shared memory), chain restarts
+                acc64[0][lane] += (double)f.x.x; acc64[1][lane] += (double)f.y.x; acc64[2][lane] += (double)f.z.x;
+                acc64[3][lane] += (double)f.x.y; acc64[4][lane] += (double)f.y.y; acc64[5][lane] += (double)f.z.y;
+                if (DENS) { acc64[6][lane] += (double)f.rho.x; acc64[7][lane] += (double)f.rho.y; }
+                f.clear();
+            };
+            if (d.flat) {
+                // Sparse window (a handful of slots per cell): a lane's 2R+1 stencil cells of this column are ONE contiguous
+                // run of quads in the stage, walked in one loop with the cell's z corner looked up per quad -- instead of
+                // 2R+1 steps that each pay ~50 instructions of piece lookup and warp reductions for one or two quads.  Lanes
+                // of different sink cells read different quads (a few shared-memory wavefronts per load, far from a limit
+                // here).  Every consumer warp fills the table of the stages it works on (same values: no ordering needed).
+                double *qz = sm.quadz[stage];
+                for (int i = lane; i < np; i += 32) {
+                    const Piece pc = d.pieces[i];
+                    for (int q = pc.sm_off >> 2, qe = (pc.sm_off + pc.nslots) >> 2; q < qe; q++) qz[q] = pc.czs;
+                }
+                if (lane == 0) qz[kTile / 4] = oczs;                 // the dummy quad: any finite corner
+                __syncwarp();
+                const int ilo = max(ibase, 0), ihi = min(ibase + 2 * R, np - 1);
+                int qlo = 0, cnt = 0;
+                if (ilo <= ihi) {
+                    const Piece pl = d.pieces[ilo], ph = d.pieces[ihi];
+                    qlo = pl.sm_off >> 2;
+                    cnt = ((ph.sm_off + ph.nslots) >> 2) - qlo;
+                }
+                const int cmax = __reduce_max_sync(kFull, cnt);
+                const bool soft = soft_mode == 2 || soft_mode == 1;     // near column: the vote decides per quad pair
+                const bool dens = DENS && (a.dens_mode == 2 || gap_dens);
+                const float4 *py0 = sbase + kTileAlloc / 4, *pz0 = py0 + kTileAlloc / 4, *pm0 = pz0 + kTileAlloc / 4;
+                const float4 one = make_float4(1.f, 1.f, 1.f, 1.f);
+                auto body = [&](auto mode) {
+                    constexpr int MODE = decltype(mode)::value;
+#pragma unroll 2
+                    for (int it = 0; it < cmax; it++) {
+                        const int q = it < cnt ? qlo + it : kTile / 4;
+                        const float dzc = (float)(qz[q] - oczs);
+                        const float2 nz = make_float2(dzc - zi.x, dzc - zi.y);
+                        quad<PACKED, MODE, MASS>(sbase[q], py0[q], pz0[q], MASS ? pm0[q] : one, nx, ny, nz, coef, f);
+                    }
+                };
+                if (DENS && dens) body(std::integral_constant<int, 2>());
+                else if (soft)    body(std::integral_constant<int, 1>());
+                else              body(std::integral_constant<int, 0>());
+                __syncwarp();
+            } else
             // Step s pairs the lanes of the warp by SOURCE cell: a lane takes the one cell j of its stencil with
             // (j - (z0 - R)) mod (2R+1) == s.  Lanes of different sink cells then read the same piece in all steps but
             // the few where the stencils do not overlap (cells j and j + 2R+1 share a step), so the piece lengths of
@@ -574,40 +669,38 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                     if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
                 if (DENS && dens) piece_loop<PACKED, 2, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
-                else if (soft)    piece_loop<PACKED, 1, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                else if (soft)    piece_loop<PACKED, 1, MASS, QV>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
                 else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                // The FP32 chain of a sink runs over ONE source cell (one step), then joins the FP64 sums: on inputs whose
+                // pair forces nearly cancel (config 2, a barely perturbed lattice) the rounding of a chain grows with its
+                // length (error ~ 2^-24 x terms x |term| / sqrt 2), and chains of a whole stage (~350 sources) put the 99.9 %
+                // quantile of the full particle set at 1.36e-5 (4.6e-6 with per-cell chains).  Steps of a few quads (sparse
+                // cells) keep adding to the same chain.
+                if (nmax >= kFlushQuads) { flush(); pending = false; } else pending = true;
             }
-            axA += (double)f.x.x; ayA += (double)f.y.x; azA += (double)f.z.x;
-            axB += (double)f.x.y; ayB += (double)f.y.y; azB += (double)f.z.y;
-            if (DENS) { rhoA += (double)f.rho.x; rhoB += (double)f.rho.y; }
+            if (pending) flush();
         }
-        if ((flags & kFlagEnd) && (sp & 15u) > 1u) {          // warp-uniform, the same for every consumer warp of the CTA
-            const int nsplit = (int)(sp & 15u), ng = (int)((sp >> 4) & 15u), q = (int)((sp >> 8) & 15u);
-            if (warp_on && q > 0) {
-                sm.part[warp][0][lane] = axA; sm.part[warp][1][lane] = ayA; sm.part[warp][2][lane] = azA;
-                sm.part[warp][3][lane] = axB; sm.part[warp][4][lane] = ayB; sm.part[warp][5][lane] = azB;
-                if (DENS) { sm.part[warp][6][lane] = rhoA; sm.part[warp][7][lane] = rhoB; }
-            }
+        if ((flags & kFlagEnd) && (sp & 255u) > 1u) {          // warp-uniform, the same for every consumer warp of the CTA
+            const int nsplit = (int)(sp & 255u), ng = (int)((sp >> 8) & 255u), q = (int)((sp >> 16) & 255u);
             asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");
             if (warp_on && q == 0) {
                 for (int t = 1; t < nsplit; t++) {
                     const int w2 = warp + t * ng;
-                    axA += sm.part[w2][0][lane]; ayA += sm.part[w2][1][lane]; azA += sm.part[w2][2][lane];
-                    axB += sm.part[w2][3][lane]; ayB += sm.part[w2][4][lane]; azB += sm.part[w2][5][lane];
-                    if (DENS) { rhoA += sm.part[w2][6][lane]; rhoB += sm.part[w2][7][lane]; }
+#pragma unroll
+                    for (int c = 0; c < (DENS ? 8 : 6); c++) acc64[c][lane] += sm.acc[w2][c][lane];
                 }
             }
-            asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");   // the buffer is free for the next unit
+            asm volatile("bar.sync 1, %0;" ::"r"(32 * kConsumerWarps) : "memory");   // the sums of the other warps may be zeroed for the next unit
         }
-        if ((flags & kFlagEnd) && nreal && ((sp >> 8) & 15u) == 0u) {
+        if ((flags & kFlagEnd) && nreal && ((sp >> 16) & 255u) == 0u) {
             const double s2 = a.k.out_scale;
 #pragma unroll
             for (int h = 0; h < 2; h++) {
                 if ((uint32_t)h >= nreal) break;
                 const size_t i = __ldg(a.perm + slot + h);
-                const float fx = (float)((h ? axB : axA) * s2), fy = (float)((h ? ayB : ayA) * s2), fz = (float)((h ? azB : azA) * s2);
+                const float fx = (float)(acc64[3 * h + 0][lane] * s2), fy = (float)(acc64[3 * h + 1][lane] * s2), fz = (float)(acc64[3 * h + 2][lane] * s2);
                 if (!EPI || a.acc) { a.acc[3 * i + 0] = fx; a.acc[3 * i + 1] = fy; a.acc[3 * i + 2] = fz; }
-                if (DENS) a.rho[i] = (float)(h ? rhoB : rhoA);
+                if (DENS) a.rho[i] = (float)acc64[6 + h][lane];
                 if (EPI && a.vel) {                                   // kick: v += a dt (leapfrog)
                     a.vel[3 * i + 0] = fmaf(fx, a.dt, a.vel[3 * i + 0]);
                     a.vel[3 * i + 1] = fmaf(fy, a.dt, a.vel[3 * i + 1]);
@@ -623,7 +716,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI, bool MASS>
+template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV = false>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
     constexpr int NARR = MASS ? 4 : 3;
@@ -639,7 +732,7 @@ __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(co
     }
     __syncthreads();
     if (warp == kConsumerWarps) producer<NARR>(a, sm, lane);
-    else                        consumer<PACKED, DENS, EPI, MASS>(a, sm, warp, lane);
+    else                        consumer<PACKED, DENS, EPI, MASS, QV>(a, sm, warp, lane);
 }
 
 typedef void (*direct_fn)(const AccelArgs);
@@ -649,8 +742,15 @@ static direct_fn pick_kernel_m(int variant, bool dens, bool epi)    // dens and 
     if (variant == 0) return dens ? direct_kernel<true, true, false, MASS> : (epi ? direct_kernel<true, false, true, MASS> : direct_kernel<true, false, false, MASS>);
     return dens ? direct_kernel<false, true, false, MASS> : (epi ? direct_kernel<false, false, true, MASS> : direct_kernel<false, false, false, MASS>);
 }
-static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false)
+static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false, bool qv = false)
 {
+    // the quad-vote instances exist for the packed force-only kernels (plain and fused epilogue, with and without masses:
+    // which pairs next to eps_s see the spline's min depends on the vote granularity, at the level of one ulp of that
+    // pair, so the mass kernel must follow the plain one for "all masses 1 = the same bits")
+    if (qv && variant == 0 && !dens) {
+        if (mass) return epi ? direct_kernel<true, false, true, true, true> : direct_kernel<true, false, false, true, true>;
+        return epi ? direct_kernel<true, false, true, false, true> : direct_kernel<true, false, false, false, true>;
+    }
     return mass ? pick_kernel_m<true>(variant, dens, epi) : pick_kernel_m<false>(variant, dens, epi);
 }
 static size_t smem_bytes(bool mass) { return mass ? sizeof(SharedStorageT<4>) : sizeof(SharedStorageT<3>); }
@@ -676,7 +776,8 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     const bool dens = rho != nullptr;
     const bool mass = p->have_mass;
     const size_t smem = smem_bytes(mass);
-    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr, mass);
+    p->quad_vote = p->quad_vote_opt >= 0 ? p->quad_vote_opt : (p->max_count > kQuadVoteAbove ? 1 : 0);
+    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr, mass, p->quad_vote != 0);
     int per_sm = 0;
     NF_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, smem) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }

@@ -34,6 +34,14 @@ constexpr int kTile          = NF_TILE;           // source slots per pipeline s
 constexpr int kStages        = NF_STAGES;         // TMA pipeline depth (three staged arrays)
 constexpr int kStagesMass    = NF_STAGES_MASS;    //   with the fourth array of the mass kernels
 constexpr int kMaxPieces     = 40;                // source cells (table entries) per stage
+#ifndef NF_QUAD_VOTE_ABOVE
+#define NF_QUAD_VOTE_ABOVE 4096
+#endif
+constexpr unsigned kQuadVoteAbove = NF_QUAD_VOTE_ABOVE;   // fullest cell above this: launch the quad-vote instance of the direct kernel
+#ifndef NF_FLAT_BELOW
+#define NF_FLAT_BELOW 14
+#endif
+constexpr int kFlatBelow     = NF_FLAT_BELOW;     // default of the "flat_below" option (padded slots per spanned cell)
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp
 constexpr int kMinCtasPerSm  = NF_MIN_CTAS;       // register budget: 65536 / (kMinCtasPerSm * kAccelThreads) per thread
 #ifndef NF_WAIT_SLEEP_NS
@@ -67,7 +75,7 @@ struct Unit {            // one work unit: a window of <= kChunk consecutive PAD
     uint32_t col;        // column id cx * cpd + cy
     uint16_t np;         // padded slots in the window, a multiple of 4
     uint16_t z0, z1;     // first and last cell (z index) that hold a slot of the window
-    uint16_t pad_;
+    uint16_t flat;       // 1: sparse window (few slots per cell): the direct kernel walks a lane's stencil run in one flat loop
 };
 
 struct Workspace {       // carved out of one arena; all 256-byte aligned
@@ -81,7 +89,8 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
     uint32_t *bucket_hist;                        // [64] + cursor
     unsigned long long *interactions;             // [1]
     uint32_t *scalars;                            // [64]: 0 error flag, 1 unit counter, 2 n_units, 3 padded total,
-                                                  //       4 movers of the last nf_rebin, 5 rebin fallback flag, 6 look-back ticket
+                                                  //       4 movers of the last nf_rebin, 5 rebin fallback flag, 6 look-back ticket,
+                                                  //       7 particles in the fullest cell
     // incremental re-binning (nf_rebin)
     uint32_t *offset_new;                         // [C+2]
     uint32_t *arr_count, *arr_off, *arr_cursor;   // [C+2] arrivals per cell, their exclusive scan, fill cursors
@@ -95,6 +104,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
 struct Consts {          // everything the kernels need about the problem, by value
     int cpd, R;
     int chunk;                      // sink slots per work unit (window of one z-column), 64..kChunk
+    int flat_below;                 // windows with fewer padded slots per spanned cell than this take the flat loop (0: none)
     int slab0, nslab;               // sink slabs: cells with x index in {slab0, ..., slab0 + nslab - 1} mod cpd (default: all)
     uint32_t ncells;
     double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L
@@ -135,6 +145,9 @@ struct nf_plan {
     float *pos_stage; float *acc_stage; size_t stage_cap;   // device staging for *_host calls
     // options
     int variant, fastpath, heavy_first, ctas_per_sm, window;
+    int quad_vote_opt;              // option "quad_vote": -1 automatic (heavy cells), 0 never, 1 always
+    int quad_vote;                  // the choice for the current binning
+    unsigned max_count;             // particles in the fullest cell of the current binning
     // stats
     cudaEvent_t ev[4];
     bool have_bin_time, have_accel_time;

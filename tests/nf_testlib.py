@@ -15,7 +15,7 @@ TOL_MAX = 1e-3    # ... and at the maximum
 # The first three are worst cases per term, the last is the random walk of the chain; measured worst ratios are printed
 # at the end of the run (conftest.py) and recorded in DESIGN.md 5.
 C13 = 2.0e-6
-RATIOS = []       # (what, worst |err| / S over the rows that miss the 1e-5 rule, their number, rows, worst |err| / S of all rows)
+RATIOS = []       # (what, worst |err| / S of the rows accepted by C13, their number, rows, rows in the 0.1 % tail, worst rel. error there)
 
 
 def u32(t: torch.Tensor) -> np.ndarray:
@@ -70,15 +70,17 @@ def assert_parity_conditioned(a_gpu, a_ref, scale, what=""):
     loose = (err <= TOL_MAX * den) | cond
     ratio = err / np.where(scale > 0, scale, 1.0)
     ratio[(scale == 0) & (err == 0)] = 0.0
-    on_c13 = ~(err <= TOL_P999 * den)                   # rows BASELINE.json's 1e-5 does not cover: judged by C13 x S
-    worst = float(ratio[on_c13].max()) if on_c13.any() else 0.0
-    RATIOS.append((what, worst, int(on_c13.sum()), len(err), float(ratio.max())))
+    outside = ~(err <= TOL_P999 * den)                  # rows BASELINE.json's 1e-5 does not cover
+    by_c13 = outside & cond                             #   ... accepted by the C13 x S bound (ill-conditioned rows)
+    tail = outside & ~cond                              #   ... accepted by neither: the 0.1 % the 99.9 % rule allows (max 1e-3)
+    worst = float(ratio[by_c13].max()) if by_c13.any() else 0.0
+    rel_all = err / np.where(den > 0, den, np.inf)
+    RATIOS.append((what, worst, int(by_c13.sum()), len(err), int(tail.sum()), float(rel_all[tail].max()) if tail.any() else 0.0))
     assert tight.mean() >= 0.999, (f"{what}: {(~tight).sum()} of {len(err)} rows miss both 1e-5 |a_ref| and C13 S "
                                    f"(worst err/S {worst:.3e})")
     assert loose.all(), f"{what}: {(~loose).sum()} rows miss both 1e-3 |a_ref| and C13 S (worst err/S {worst:.3e})"
-    rel = err / np.where(den > 0, den, np.inf)
-    return {"p999": float(np.quantile(rel, 0.999)), "max": float(rel.max()), "worst_ratio": worst,
-            "rows_on_C13": int((~(err <= TOL_P999 * den)).sum())}
+    return {"p999": float(np.quantile(rel_all, 0.999)), "max": float(rel_all.max()), "worst_ratio": worst,
+            "rows_on_C13": int(by_c13.sum()), "rows_in_tail": int(tail.sum())}
 
 
 def assert_binning_equal(b_gpu: dict, b_ref: dict):

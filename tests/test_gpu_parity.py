@@ -560,7 +560,8 @@ def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, worl
     pos_d = pos.cuda()
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
         plan.set_option("window", 64)       # any window: equal on every plan
-        plan.bin(pos_d)
+        plan.set_option("quad_vote", idx % 2)   # any instance of the direct kernel: equal on every plan (the automatic choice
+        plan.bin(pos_d)                         # looks at the fullest cell a plan holds, which differs between the ranks)
         whole = plan.accel().cpu()
         total = plan.stats()["interactions"]
         cost = plan.slab_cost()
@@ -586,6 +587,7 @@ def test_slab_decomposition_matches_whole_box(oracle_mod, idx, n_side, cpd, worl
         with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as plan:
             plan.set_sink_slabs(f, c)
             plan.set_option("window", 64)
+            plan.set_option("quad_vote", idx % 2)
             plan.bin(local)
             acc = torch.full((local.shape[0], 3), 7.0, device="cuda")
             plan.accel(acc)
@@ -767,6 +769,7 @@ def test_masses_fused_passes_and_errors(oracle_mod):
     b = 0.4 / cfg.n_side
     with nf.Plan(cfg.cpd, cfg.L, cfg.eps, cfg.R) as p:
         p.n = cfg.n
+        p.set_option("quad_vote", 0)        # one vote granularity in every entry point: then the forces agree bit for bit
         with pytest.raises(nf.NFError):
             p.set_masses(mass.cuda())                                       # before nf_bin
         p.bin(pos.cuda())
@@ -1006,3 +1009,26 @@ def test_rebin_full_size(oracle_mod, idx, device):
             _, b, st = _rebin_check(oracle_mod, plan, pos, cfg, f"{cfg.name} rebin {step}", expect_path=1, fresh=(step == 1))
             print(f"{cfg.name}: nf_bin {ms_full:.3f} ms, nf_rebin {st['ms_bin']:.3f} ms with {st['rebin_movers']} movers "
                   f"({100.0 * st['rebin_movers'] / cfg.n:.2f} %)")
+
+
+# ---------------------------------------------------------------- sparse windows: the flat loop of the direct kernel
+@pytest.mark.parametrize("n,cpd,R,flat_below", [(8000, 10, 2, 14), (8000, 16, 2, 14), (6000, 20, 2, 14), (8000, 16, 2, 0), (20000, 12, 3, 1024),
+                                                (30000, 9, 2, 1024), (3000, 25, 1, 14)])
+def test_sparse_flat_loop(oracle_mod, n, cpd, R, flat_below):
+    """Windows with a handful of slots per cell walk a lane's stencil run in one flat loop (nf_set_option "flat_below"):
+    8, 2 and 0.75 particles per cell with the default threshold, the same grid with the flat loop switched off, and dense
+    grids FORCED onto the flat loop (threshold 1024) -- all against the oracle; voids and a clump in the same box."""
+    g = torch.Generator().manual_seed(n + cpd)
+    pos = torch.rand((n, 3), generator=g)
+    pos[: n // 10] = 0.37 + 0.002 * torch.randn((n // 10, 3), generator=g)          # a clump: heavy cells next to sparse windows
+    pos = torch.remainder(pos, 1.0).to(torch.float32).contiguous()
+    pos[pos >= 1.0] = 0.0
+    st, out = full_check(oracle_mod, pos, cpd, 1.0, 0.01 / cpd, R, options={"flat_below": flat_below}, what=f"flat n={n} cpd={cpd} R={R}")
+    import paper_2110_11398_b200 as nf
+    with nf.Plan(cpd, 1.0, 0.01 / cpd, R) as plan:                                   # fused passes on the same path
+        plan.set_option("flat_below", flat_below)
+        plan.bin(pos.cuda())
+        acc, rho = plan.accel_density(0.4 / cpd)
+        ref_rho = oracle_mod.density(pos.numpy(), cpd, 1.0, 0.4 / cpd, R)
+        assert (np.abs(rho.cpu().numpy().astype(np.float64) - ref_rho) / ref_rho).max() <= 1e-5
+        assert (acc.cpu().double().numpy() - out["acc"]).__abs__().max() <= 1e-5 * np.abs(out["acc"]).max()

@@ -202,6 +202,19 @@ int nf_set_sink_slabs(nf_plan *plan, int x_first, int n_slabs);
  *   1 <= world <= cpd and every cost is finite and >= 0.
  */
 int nf_slab_histogram(nf_plan *plan, const float *pos_dev, long long n, long long *hist_host);
+/*
+ * nf_slab_histogram_static -- nf_slab_histogram (same arguments, same result, same errors) for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  The scratch of the
+ * kernel (per-slab counters and the domain flag) is a file-scope device array of the library, not an allocation: the
+ * call makes no cudaMalloc / cudaFree, calls no allocating library routine and uses no host heap.
+ *   limit    cpd <= 1024 (the array holds 1024 slab counters + the flag: 8 KB, held by every GPU that loads the library
+ *            until the process exits); a larger cpd -> NF_ERR_ARG with a message naming the limit.
+ *   sharing  every call on a device uses the ONE array, which keeps the previous call's contents (the call clears what it
+ *            uses first).  Calls that overlap on the same GPU -- other streams, other plans, other host threads -- RACE:
+ *            the caller serialises them.  nf_slab_histogram has no such restriction.
+ * Runs on the plan's device if it has one (bound at its first nf_bin), else on the current device.  Synchronises.
+ */
+int nf_slab_histogram_static(nf_plan *plan, const float *pos_dev, long long n, long long *hist_host);
 int nf_slab_select(nf_plan *plan, const float *pos_dev, long long n, int x_first, int n_slabs, float *out_dev,
                    unsigned *idx_out_dev, long long cap, long long *m_host);
 int nf_get_slab_cost(nf_plan *plan, double *cost_host);

@@ -24,7 +24,7 @@ EXPORTS = [
     "nf_plan_create", "nf_bin", "nf_rebin", "nf_accel", "nf_accel_density", "nf_accel_kick", "nf_set_masses", "nf_set_sink_slabs", "nf_destroy", "nf_bin_host", "nf_accel_host",
     "nf_last_error", "nf_set_stream", "nf_workspace_bytes", "nf_set_workspace", "nf_get_binning",
     "nf_get_layout", "nf_get_stats", "nf_set_option",
-    "nf_slab_histogram", "nf_slab_select", "nf_get_slab_cost", "nf_slab_partition",
+    "nf_slab_histogram", "nf_slab_select", "nf_get_slab_cost", "nf_slab_partition", "nf_slab_histogram_static",
 ]
 
 
@@ -101,6 +101,8 @@ def _load() -> ctypes.CDLL:
     lib.nf_set_option.argtypes = [vp, ctypes.c_char_p, ll]
     lib.nf_slab_histogram.restype = i32
     lib.nf_slab_histogram.argtypes = [vp, vp, ll, ctypes.POINTER(ll)]
+    lib.nf_slab_histogram_static.restype = i32
+    lib.nf_slab_histogram_static.argtypes = [vp, vp, ll, ctypes.POINTER(ll)]
     lib.nf_slab_select.restype = i32
     lib.nf_slab_select.argtypes = [vp, vp, ll, i32, i32, vp, vp, ll, ctypes.POINTER(ll)]
     lib.nf_get_slab_cost.restype = i32
@@ -262,6 +264,15 @@ def nf_slab_histogram(plan: int, pos: torch.Tensor, cpd: int) -> list[int]:
     pos = _dev_f32(pos, "pos")
     h = (ctypes.c_longlong * cpd)()
     _check(_lib.nf_slab_histogram(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0], h))
+    return list(h)
+
+
+def nf_slab_histogram_static(plan: int, pos: torch.Tensor, cpd: int) -> list[int]:
+    """nf_slab_histogram without any allocation on the device side: scratch in a static device array of the library
+    (cpd <= 1024; calls that overlap on one GPU race -- include/nf.h)."""
+    pos = _dev_f32(pos, "pos")
+    h = (ctypes.c_longlong * cpd)()
+    _check(_lib.nf_slab_histogram_static(plan, ctypes.c_void_p(pos.data_ptr()), pos.shape[0], h))
     return list(h)
 
 

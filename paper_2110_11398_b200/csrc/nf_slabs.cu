@@ -242,3 +242,81 @@ int nf_slab_partition(const double *cost, int cpd, int world, int *first, int *c
 }
 
 }  // extern "C"
+
+// ==================================================================================================================
+// nf_slab_histogram_static -- nf_slab_histogram for callers that must not allocate (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc): the same kernel, its scratch (the per-slab counters and the
+// domain flag) in a file-scope device array instead of a cudaMalloc'ed buffer.  No cudaMalloc, no cudaFree, no
+// allocating library routine, no host heap.
+//   * every GPU that loads the library holds the array (8 KB) until the process exits;
+//   * the limit is cpd <= kStaticMaxCpd (larger grids: nf_slab_histogram);
+//   * every call on a device shares the ONE array and finds the previous call's numbers in it: the call clears what
+//     it uses first, and two calls that overlap on the same GPU (other streams, other plans, other host threads) race
+//     -- the caller serialises them.
+// In host code `g_slab_scratch` is a host-side stand-in, not a device address: the device address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kStaticMaxCpd = 1024;
+static __device__ __align__(256) unsigned long long g_slab_scratch[kStaticMaxCpd + 2];   // [cpd] counts, then the flag word
+
+namespace nf {
+constexpr int kStaticMaxDevices = 64;
+static unsigned long long *g_slab_scratch_ptr[kStaticMaxDevices];        // device address of g_slab_scratch on device i (0: not asked yet)
+
+// the device address of the scratch on the CURRENT device (dev); not thread-safe against a first call on the same
+// device from another host thread beyond both storing the same value
+static int static_scratch(int dev, unsigned long long **out)
+{
+    if (dev < 0 || dev >= kStaticMaxDevices) { set_error("nf_slab_histogram_static: device %d outside [0, %d)", dev, kStaticMaxDevices); return NF_ERR_ARG; }
+    if (!g_slab_scratch_ptr[dev]) {
+        unsigned long long *ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_slab_scratch);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            set_error("nf_slab_histogram_static: cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+            return NF_ERR_CUDA;
+        }
+        g_slab_scratch_ptr[dev] = ptr;
+    }
+    *out = g_slab_scratch_ptr[dev];
+    return NF_OK;
+}
+}  // namespace nf
+
+extern "C" int nf_slab_histogram_static(nf_plan *p, const float *pos, long long n, long long *hist_host)
+{
+    if (!p || !hist_host || n < 0 || (!pos && n > 0)) { set_error("nf_slab_histogram_static: bad argument"); return NF_ERR_ARG; }
+    const int cpd = p->k.cpd;
+    if (cpd > kStaticMaxCpd) {
+        set_error("nf_slab_histogram_static: cpd = %d exceeds the static scratch (at most %d slabs); use nf_slab_histogram", cpd, kStaticMaxCpd);
+        return NF_ERR_ARG;
+    }
+    for (int s = 0; s < cpd; s++) hist_host[s] = 0;
+    if (n == 0) return NF_OK;
+    // the plan's device if it has one (bound at its first nf_bin), else the current one; current for the rest of the call
+    int cur = -1, prev = -1;
+    NF_CUDA_OK(cudaGetDevice(&cur));
+    if (p->device >= 0 && p->device != cur) { NF_CUDA_OK(cudaSetDevice(p->device)); prev = cur; cur = p->device; }
+    unsigned long long *d = nullptr;
+    int rc = nf::static_scratch(cur, &d);
+    unsigned long long flag = 0;
+    cudaError_t e = cudaSuccess;
+    if (rc == NF_OK) {
+        cudaStream_t st = p->stream;
+        e = cudaMemsetAsync(d, 0, 8 * (size_t)(cpd + 1), st);                   // the array keeps the last call's contents
+        if (e == cudaSuccess) {
+            const size_t want = ((size_t)n + kSelThreads - 1) / kSelThreads;
+            const unsigned grid = (unsigned)(want < 2048 ? want : 2048);
+            slab_hist_kernel<<<grid, kSelThreads, 4 * (size_t)cpd, st>>>(pos, (size_t)n, p->k, d, reinterpret_cast<uint32_t *>(d + cpd));
+            e = cudaGetLastError();
+        }
+        // counts are below 2^63: the bits of unsigned long long ARE the caller's long long
+        if (e == cudaSuccess) e = cudaMemcpyAsync(hist_host, d, 8 * (size_t)cpd, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&flag, d + cpd, 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    if (prev >= 0) cudaSetDevice(prev);
+    if (rc != NF_OK) return rc;
+    if (e != cudaSuccess) { set_error("nf_slab_histogram_static: %s", cudaGetErrorString(e)); return NF_ERR_CUDA; }
+    if (flag & 1ull) { set_error("nf_slab_histogram_static: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
+    return NF_OK;
+}

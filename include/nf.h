@@ -270,7 +270,7 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *   "fastpath"     1 = skip the spline on cells that cannot hold a pair closer than eps_s (default), 0 = never skip
  *   "heavy_first"  1 = schedule costly work units first (default), 0 = natural cell order
  *   "ctas_per_sm"  0 = occupancy-derived (default), >0 = cap
- *   "window"       sink slots (padded: cells are padded to multiples of 4) per work unit: a multiple of 32 up to 512, rounded
+ *   "window"       sink slots (the particles of a z-column, every cell rounded up to an even count) per work unit: a multiple of 32 up to 512, rounded
  *                  up to whole sink groups of 64, or 0 (default) = 512, except for problems whose units would not fill the
  *                  grid of persistent CTAs, which get the longest of 512, 256, 128 and 64 that does.
  *                  The warps of a CTA that a short window leaves without sinks share the unit's stages.
@@ -284,8 +284,9 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *                  launched when the fullest cell of the binning holds more than 4096 particles (the halo cells of clustered
  *                  inputs spend nearly all their pairs in that loop); 0 = never, 1 = always.  The two instances agree to one ulp of the
  *                  pairs that sit within 0.1 % of eps_s (the spline's min is taken wherever the vote fired): bit-identical
- *                  results between plans (slab ranks against the whole box) or between nf_accel and the fused
- *                  nf_accel_density pass (which always votes per two sources) need the same explicit setting.
+ *                  results between plans (slab ranks against the whole box) need the same explicit setting.  The fused
+ *                  nf_accel_density pass votes on max(eps_s, b): its forces agree with nf_accel's to that one ulp, not bit
+ *                  for bit; nf_accel_kick runs the loops of nf_accel and returns its bits.
  *   "softening"    0 = the compact spline of the method (default); 1 = Plummer softening, force
  *                  d (r^2 + eps^2)^(-3/2) with eps the plan's length: the law the paper compares against
  *                  ("converges only quadratically to the correct large-scale force law")

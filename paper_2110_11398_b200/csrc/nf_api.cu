@@ -56,6 +56,7 @@ size_t carve(Workspace &ws, void *base, long long n, int cpd)
     ws.scalars      = (uint32_t *)take(4 * 64);
     ws.offset = (uint32_t *)take(4 * (C + 2));
     ws.poff   = (uint32_t *)take(4 * (C + 2));
+    ws.voff   = (uint32_t *)take(4 * (C + 2));
     ws.ubase  = (uint32_t *)take(4 * (C + 2));
     ws.src    = (uint32_t *)take(4 * (C + 1));
     ws.scan_tmp = (uint32_t *)take(4 * (scan_items / 2048 + 4096));

@@ -50,6 +50,7 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *t
 // ---- three-kernel exclusive scan with an element transform -----------------------------------
 struct OpId    { __device__ uint32_t operator()(uint32_t v) const { return v; } };
 struct OpPad4  { __device__ uint32_t operator()(uint32_t v) const { return (v + 3u) & ~3u; } };
+struct OpPad2  { __device__ uint32_t operator()(uint32_t v) const { return (v + 1u) & ~1u; } };
 
 constexpr int kScanThreads = 256, kScanItems = 8, kScanTile = kScanThreads * kScanItems;
 
@@ -134,13 +135,15 @@ __global__ void __launch_bounds__(kSmallThreads) scan_small(const uint32_t *in, 
 
 // Small problems are bound by the number of launches of nf_bin: the three prefix sums that follow the cell-id kernel
 // (cell offsets, padded offsets, the digit histogram of the single sort pass) in one launch.
-__global__ void __launch_bounds__(kSmallThreads) small_scans_kernel(const uint32_t *count, uint32_t *offset, uint32_t *poff, uint32_t ncells,
-                                                                    uint32_t *hist, uint32_t nhist, uint32_t *padded_total)
+__global__ void __launch_bounds__(kSmallThreads) small_scans_kernel(const uint32_t *count, uint32_t *offset, uint32_t *poff, uint32_t *voff,
+                                                                    uint32_t ncells, uint32_t *hist, uint32_t nhist, uint32_t *padded_total)
 {
     __shared__ uint32_t sm[33];
     scan_small_body(count, offset, ncells, OpId(), 1, nullptr, sm);
     __syncthreads();
     scan_small_body(count, poff, ncells, OpPad4(), 1, padded_total, sm);
+    __syncthreads();
+    scan_small_body(count, voff, ncells, OpPad2(), 1, nullptr, sm);
     __syncthreads();
     scan_small_body(hist, hist, nhist, OpId(), 0, nullptr, sm);
 }
@@ -511,8 +514,9 @@ __global__ void __launch_bounds__(256) cellcost_kernel(Consts k, const uint32_t 
     }
 }
 
-// work units per z-column: windows of k.chunk consecutive PADDED slots (sink slots; a lane of the direct kernel holds an
-// aligned pair of them, and cells are padded to multiples of 4 slots, so a pair never straddles two cells).
+// work units per z-column: windows of k.chunk consecutive SINK slots (the particles of a column numbered with every cell
+// rounded up to an even count, voff: a lane of the direct kernel holds an aligned pair of them, which never straddles two
+// cells; only the last slot of a cell with an odd count is an idle sink).
 // Length of the next window of a column that has `rem` slots left.  Whole windows of `chunk`; the remainder of a
 // column with default windows is cut so that its sink groups (64 slots each) divide the consumer warps: 5-7 groups ->
 // 256 slots (4 groups) first, 3 groups -> 128 slots (2 groups) first.  Every window then keeps all the warps of its CTA
@@ -534,24 +538,24 @@ __device__ __forceinline__ uint32_t windows_in(uint32_t ncol, uint32_t chunk)
     return nw;
 }
 
-__global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ poff,
+__global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t *__restrict__ voff,
                                                        uint32_t *__restrict__ nunits)
 {
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
-    const uint32_t ncol = poff[(size_t)(col + 1) * k.cpd] - poff[(size_t)col * k.cpd];
+    const uint32_t ncol = voff[(size_t)(col + 1) * k.cpd] - voff[(size_t)col * k.cpd];
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
     nunits[col] = rel < k.nslab ? windows_in(ncol, (uint32_t)k.chunk) : 0u;      // columns outside the sink slabs: sources only
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
-__global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ poff, const uint32_t *__restrict__ count,
+__global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ voff, const uint32_t *__restrict__ count,
                                                     const uint32_t *__restrict__ src, const uint32_t *__restrict__ ubase,
                                                     Unit *__restrict__ units, uint32_t *__restrict__ ukey)
 {
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
-    const uint32_t *off = poff + (size_t)col * k.cpd;
+    const uint32_t *off = voff + (size_t)col * k.cpd;
     const uint32_t *cn = count + (size_t)col * k.cpd;
     const uint32_t *sc = src + (size_t)col * k.cpd;
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
@@ -564,7 +568,7 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
         const uint32_t s1 = s0 + len;
         while (off[z + 1] <= s0) z++;                     // cell holding slot s0 (skips empty cells)
         Unit un;
-        un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
+        un.v0 = s0; un.col = col; un.nv = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
         unsigned long long cost = 0;                      // exact pair interactions of the window's real sinks
         int zz = z;
         for (;;) {
@@ -574,7 +578,7 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
             zz++;
         }
         un.z1 = (uint16_t)zz;
-        un.flat = (uint16_t)((uint32_t)un.np < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
+        un.flat = (uint16_t)((uint32_t)un.nv < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
         units[u] = un;
         ukey[u] = (uint32_t)__clzll((long long)cost);     // heavier -> smaller key
         z = zz;
@@ -615,7 +619,7 @@ int launch_set_masses(nf_plan *p, const float *mass)
 // column, heavy-first order by a counting sort on the cost key (not stable: the order of equal keys only matters for L2
 // locality, which a problem of this size has anyway; no result depends on the unit order).
 constexpr int kSmallCells = 2048, kSmallUnits = 4096;
-__global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint32_t *__restrict__ count, const uint32_t *__restrict__ poff,
+__global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint32_t *__restrict__ count, const uint32_t *__restrict__ voff,
                                                            uint32_t *__restrict__ src_out, unsigned long long *__restrict__ interactions,
                                                            Unit *__restrict__ units, Unit *__restrict__ units_sorted,
                                                            uint32_t *__restrict__ scalars, int heavy_first)
@@ -629,7 +633,7 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
     for (uint32_t c = threadIdx.x; c < C; c += 1024) { s_cnt[c] = count[c]; cmax = max(cmax, s_cnt[c]); }
     cmax = __reduce_max_sync(0xffffffffu, cmax);
     if ((threadIdx.x & 31) == 0 && cmax) atomicMax(&scalars[7], cmax);
-    for (uint32_t c = threadIdx.x; c <= C; c += 1024) s_off[c] = poff[c];
+    for (uint32_t c = threadIdx.x; c <= C; c += 1024) s_off[c] = voff[c];
     if (threadIdx.x < 66) { s_hist[threadIdx.x] = 0; s_cur[threadIdx.x] = 0; }
     if (threadIdx.x == 0) s_inter = 0;
     __syncthreads();
@@ -653,7 +657,9 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
         int rel = cx - k.slab0; rel += rel < 0 ? cpd : 0;
         if (rel < k.nslab) mine += (unsigned long long)s_cnt[c] * src;      // sinks of the owned slabs only
     }
-    if (mine) atomicAdd(&s_inter, mine);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(0xffffffffu, mine, o);     // one 64-bit shared atomic per warp, not per cell
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&s_inter, mine);
     __syncthreads();
     for (uint32_t col = threadIdx.x; col < ncols; col += 1024) {
         const uint32_t ncol = s_off[(col + 1) * cpd] - s_off[col * cpd];
@@ -688,7 +694,7 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
             const uint32_t s1 = s0 + len;
             while (off[z + 1] <= s0) z++;
             Unit un;
-            un.p0 = s0; un.col = col; un.np = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
+            un.v0 = s0; un.col = col; un.nv = (uint16_t)(s1 - s0); un.z0 = (uint16_t)z; un.flat = 0;
             unsigned long long cost = 0;
             int zz = z;
             for (;;) {
@@ -698,7 +704,7 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
                 zz++;
             }
             un.z1 = (uint16_t)zz;
-            un.flat = (uint16_t)((uint32_t)un.np < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
+            un.flat = (uint16_t)((uint32_t)un.nv < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
             units[u] = un;
             const uint32_t key = (uint32_t)__clzll((long long)cost);
             s_key[u] = (unsigned char)key;
@@ -744,14 +750,14 @@ static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free
     const uint32_t ncols = (uint32_t)k.cpd * (uint32_t)k.cpd;
     uint32_t *ukey = (uint32_t *)ws.units_sorted;
     cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions, &ws.scalars[7]);  L++;
-    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.poff, ws.ubase);  L++;
+    colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.voff, ws.ubase);  L++;
     exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
-    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.poff, ws.count, ws.src, ws.ubase, ws.units, ukey);  L++;
+    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.voff, ws.count, ws.src, ws.ubase, ws.units, ukey);  L++;
     NF_CUDA_OK(cudaGetLastError());
 
     // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
     const size_t ncol_sink = (size_t)k.nslab * k.cpd;
-    const size_t pmax = n + 3 * (n < (size_t)k.ncells ? n : (size_t)k.ncells);            // padded slots
+    const size_t pmax = n + (n < (size_t)k.ncells ? n : (size_t)k.ncells);                // sink slots: every non-empty cell adds at most one
     const size_t umax = (n < ncol_sink ? n : ncol_sink) + pmax / (size_t)(k.chunk < kGroup ? kGroup : k.chunk) + 2 * ncol_sink + 2;
     const size_t ucap = (n < (size_t)ncols ? n : (size_t)ncols) + n / 16 + 2;            // what carve() reserved
     const size_t ub = umax < ucap ? umax : ucap;
@@ -775,7 +781,7 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     if (p->window > 0) p->k.chunk = p->window;
     else if (n_ll > 0) {
         const double cols = (double)p->k.nslab * p->k.cpd;
-        const double per_col = 1.03 * (double)n_ll / ((double)p->k.cpd * p->k.cpd);      // padded slots, roughly
+        const double per_col = 1.01 * (double)n_ll / ((double)p->k.cpd * p->k.cpd);      // sink slots, roughly
         const double slots = (double)p->sm_count * kMinCtasPerSm;
         int w = kChunk;
         while (w > kGroup && cols * std::ceil(per_col / w) < slots) w >>= 1;    // sink-group counts that divide the consumer warps
@@ -807,10 +813,11 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
                        pmax_small / kGroup + 3 * (size_t)k.cpd * k.cpd + 2 <= (size_t)kSmallUnits;
     // prefix sums: offset (exported), padded offsets, unit bases
     if (small) {
-        small_scans_kernel<<<1, kSmallThreads, 0, st>>>(ws.count, ws.offset, ws.poff, k.ncells, ws.radix_hist, nbs << dbits, &ws.scalars[3]);  L++;
+        small_scans_kernel<<<1, kSmallThreads, 0, st>>>(ws.count, ws.offset, ws.poff, ws.voff, k.ncells, ws.radix_hist, nbs << dbits, &ws.scalars[3]);  L++;
     } else {
         exclusive_scan(ws.count, ws.offset, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
         exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
+        exclusive_scan(ws.count, ws.voff, (size_t)k.ncells, ws.scan_tmp, OpPad2(), 1, nullptr, st, &L);
     }
 
     GatherArgs g;
@@ -829,7 +836,7 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     uint32_t *free_key = kbuf[passes & 1], *free_val = vbuf[passes & 1];   // the pair not holding the result
 
     if (small) {
-        small_units_kernel<<<1, 1024, 0, st>>>(k, ws.count, ws.poff, ws.src, ws.interactions, ws.units, ws.units_sorted, ws.scalars,
+        small_units_kernel<<<1, 1024, 0, st>>>(k, ws.count, ws.voff, ws.src, ws.interactions, ws.units, ws.units_sorted, ws.scalars,
                                                p->heavy_first);  L++;
     } else {
         const int rc = launch_units(p, n, free_key, free_val, &L);
@@ -1176,6 +1183,7 @@ int launch_rebin(nf_plan *p, const float *pos)
     exclusive_scan(ws.arr_count, ws.arr_off, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
     exclusive_scan(ws.count, ws.offset_new, (size_t)k.ncells, ws.scan_tmp, OpId(), 1, nullptr, st, &L);
     exclusive_scan(ws.count, ws.poff, (size_t)k.ncells, ws.scan_tmp, OpPad4(), 1, &ws.scalars[3], st, &L);
+    exclusive_scan(ws.count, ws.voff, (size_t)k.ncells, ws.scan_tmp, OpPad2(), 1, nullptr, st, &L);
     rebin_fill_kernel<<<(cap + 255) / 256, 256, 0, st>>>(ws.mover_list, cap, ws.scalars, ws.cid, ws.arr_off, ws.arr_cursor, ws.arr_list);  L++;
     // the cells' arrival lists in ascending index: ranked by comparison, sum of (arrivals per cell)^2 operations, bounded by
     // 16 n (a 3e6-particle halo cell that exchanges 1 % of its members costs 9e8); beyond that the host sorts from scratch

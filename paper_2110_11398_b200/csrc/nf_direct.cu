@@ -5,9 +5,10 @@
 //   O(N^2) summation with a compact spline softening kernel"; periodic images kept).
 //
 // Design (sm_100a):
-//   * a work unit is a WINDOW of <= kChunk consecutive PADDED sink slots of one z-column (cells are z-fastest,
-//     so a column is one contiguous run of the source arrays): every warp holds 64 slots whatever the cell
-//     occupancy -- only the pad slots (cells are padded to multiples of 4) are idle sinks;
+//   * a work unit is a WINDOW of <= kChunk consecutive sink slots of one z-column (cells are z-fastest, so a
+//     column is one contiguous run of the sorted order; sink slots number its particles with every cell rounded
+//     up to an even count): every warp holds 64 slots whatever the cell occupancy -- only the last slot of a
+//     cell with an odd count is an idle sink;
 //   * persistent CTAs, one producer warp + kConsumerWarps consumer warps, units pulled from an atomic
 //     counter in heavy-first order;
 //   * for each of the (2R+1)^2 neighbour columns the producer streams the z-run of cells [z0-R, z1+R] that the
@@ -17,7 +18,7 @@
 //     pointer), so no lane ever evaluates a pair outside its stencil; the order pairs the lanes of a warp by
 //     source cell (step s takes the cell j with (j - z0 + R) mod (2R+1) == s), so lanes of neighbouring sink
 //     cells read the same piece except in the one step where their stencils do not overlap;
-//   * TWO sinks per lane in registers, an aligned pair of padded slots (always the same cell), packed as the two
+//   * TWO sinks per lane in registers, an aligned pair of sink slots (always the same cell), packed as the two
 //     halves of f32x2 operands; sources are read as LDS.128 of 4 x, 4 y, 4 z and every source is a scalar
 //     broadcast against the sink pair: FADD2 / FFMA2 / FMUL2 (fma.rn.f32x2) do two interactions each, one
 //     MUFU.RSQ per interaction.  Every shared-memory load, every piece lookup and every loop instruction of a
@@ -50,8 +51,8 @@ struct __align__(16) StageDesc {
     int      j0;               // cell of pieces[0], as an index relative to z0 - R
     int      soft_mode;        // 2: spline body everywhere; 1: for |oz| <= 1 (column with |ox|,|oy| <= 1); 0: never
     float    dx, dy;           // sink shift of this column: d = x_src - (x_sink - shift), scaled units
-    uint32_t p0;               // unit: first padded sink slot
-    uint32_t np;               //       padded sink slots
+    uint32_t v0;               // unit: first sink slot (voff numbering: cells rounded up to even counts)
+    uint32_t nv;               //       sink slots
     uint32_t z0, z1;           //       first / last sink cell (z index)
     uint32_t colbase;          //       col * cpd
     int      oxy;              // column offset: (ox + 128) | (oy + 128) << 8
@@ -122,7 +123,7 @@ __device__ __forceinline__ float rsqrt_approx(float x)
 // A lane holds two sinks A, B; every float2 below is (value for A, value for B).  PACKED: f32x2 instructions (FADD2, FFMA2,
 // FMUL2: two interactions each; a source coordinate enters as a scalar broadcast operand); otherwise scalar FP32 (variant 1).
 constexpr float kSelfR2 = 2e-36f;   // r^2 of a pair at r = 0 is the offset `tiny` = 1e-36 (spline law); nothing else is below this
-struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin)
+struct SoftCoef { float A, B, C, tiny, soft_r2, nb2, dens_r2; int plummer; float near_r2; };   // density: nb2 = -1/b^2, dens_r2 = b^2 (+ tiny, margin); near_r2 = max(soft_r2, dens_r2)
 
 template <bool PACKED> __device__ __forceinline__ float2 add2(const float2 a, const float2 b)
 {
@@ -154,6 +155,9 @@ constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable
 #endif
 constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
+#ifndef NF_DENS_QV
+#define NF_DENS_QV 1                           // fused density loops: one combined vote per quad (1) or two votes per two sources (0)
+#endif
 #ifndef NF_FLUSH_QUADS
 #define NF_FLUSH_QUADS 6
 #endif
@@ -240,7 +244,7 @@ template <bool PACKED, int MODE, bool MASS, bool QV = false>
 __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float4 Z, const float4 M, const float2 nx, const float2 ny,
                                      const float2 nz, const SoftCoef &c, Partial &f, const uint32_t mask = kFull)
 {
-    if (MODE != 1 || !QV) {
+    if (MODE == 0 || !QV) {
         duo<PACKED, MODE, MASS>(X.x, Y.x, Z.x, M.x, X.y, Y.y, Z.y, M.y, nx, ny, nz, c, f, mask);
         duo<PACKED, MODE, MASS>(X.z, Y.z, Z.z, M.z, X.w, Y.w, Z.w, M.w, nx, ny, nz, c, f, mask);
         return;
@@ -258,19 +262,32 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
         src_head<PACKED>(xs[j], ys[j], zs[j], nx, ny, nz, c.tiny, dx[j], dy[j], dz[j], r2, ri, k[j]);
         m = fminf(m, fminf(r2.x, r2.y));
     }
-    if (__any_sync(mask, m < c.soft_r2)) {
+    // MODE 2 (the fused density pass): ONE vote for "some lane has one of these sources inside eps_s OR inside b"; the kernel
+    // density radius b is several eps_s, so the spline gets a second vote inside the (already rare) branch.  Config 3: +7.2 %
+    // -> +4.9 % over the force-only pass; config 4: +31 % -> +25 % (in the halo cores every quad has a source within b: an
+    // unconditional density body for heavy pieces, without vote and recompute, measured the same 25 % -- the weight itself,
+    // one FFMA2, two FMNMX and one FADD2 per two interactions, is what costs there).
+    if (__any_sync(mask, m < (MODE == 2 ? c.near_r2 : c.soft_r2))) {
+        const bool spline = MODE == 1 || __any_sync(mask, m < c.soft_r2);
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             float2 r2 = fma2<PACKED>(dz[j], dz[j], bc(c.tiny));
             r2 = fma2<PACKED>(dy[j], dy[j], r2);
             r2 = fma2<PACKED>(dx[j], dx[j], r2);
-            float2 ri;
-            ri.x = rsqrt_approx(r2.x);
-            ri.y = rsqrt_approx(r2.y);
-            src_spline<PACKED>(r2, ri, c, k[j]);
-            if (MASS) {                        // see duo: drop r = 0 before the mass multiplies the capped k
-                k[j].x = r2.x > kSelfR2 ? k[j].x : 0.f;
-                k[j].y = r2.y > kSelfR2 ? k[j].y : 0.f;
+            if (spline) {
+                float2 ri;
+                ri.x = rsqrt_approx(r2.x);
+                ri.y = rsqrt_approx(r2.y);
+                src_spline<PACKED>(r2, ri, c, k[j]);
+                if (MASS) {                    // see duo: drop r = 0 before the mass multiplies the capped k
+                    k[j].x = r2.x > kSelfR2 ? k[j].x : 0.f;
+                    k[j].y = r2.y > kSelfR2 ? k[j].y : 0.f;
+                }
+            }
+            if (MODE == 2) {                   // weights of the lanes without a source inside b are exactly 0
+                if (c.plummer)                 // the Plummer option puts eps^2 into r2: the weight needs the bare r^2
+                    r2 = fma2<PACKED>(dx[j], dx[j], fma2<PACKED>(dy[j], dy[j], mul2<PACKED>(dz[j], dz[j])));
+                src_density<PACKED>(r2, c, f.rho);
             }
         }
     }
@@ -321,7 +338,7 @@ struct AccelArgs {
     Consts k;
     const float *x, *y, *z;          // padded SoA sources (= sinks)
     const float *m;                  // padded SoA source masses (MASS kernels only; pads hold 0)
-    const uint32_t *poff, *offset, *perm;
+    const uint32_t *poff, *voff, *offset, *perm;
     const Unit *units;
     uint32_t n_units;
     uint32_t *counter;               // atomic work counter (zeroed before launch)
@@ -428,7 +445,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.p0 = un.p0; d.np = un.np; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.v0 = un.v0; d.nv = un.nv; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -475,7 +492,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
                                     d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
-                                    d.p0 = un.p0; d.np = un.np; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                                    d.v0 = un.v0; d.nv = un.nv; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
                                 }
                             }
@@ -507,13 +524,14 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
 template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV>
 __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS ? 4 : 3> &sm, const int warp, const int lane)
 {
-    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f,
-                           DENS ? -1.001f / a.dens_nb2 + a.k.tiny : 0.f, a.k.plummer};
+    const float dens_r2 = DENS ? -1.001f / a.dens_nb2 + a.k.tiny : 0.f;
+    const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f, dens_r2, a.k.plummer,
+                           fmaxf(a.k.soft_r2, dens_r2)};
     constexpr int kStages = StagesFor<MASS ? 4 : 3>::value;
     const int nsteps = 2 * a.k.R + 1, R = a.k.R;
     int stage = 0;
     uint32_t phase = 0;
-    float2 xi = make_float2(0.f, 0.f), yi = xi, zi = xi;         // the lane's two sinks (A, B): an aligned pair of padded slots
+    float2 xi = make_float2(0.f, 0.f), yi = xi, zi = xi;         // the lane's two sinks (A, B): an aligned pair of sink slots
     double oczs = 0.0;
     double (*acc64)[32] = sm.acc[warp];                          // [8][32]: this warp's FP64 sums, one column per lane
     // A window of fewer than kChunk slots leaves consumer warps without sinks.  They take a share of the unit's stages
@@ -535,37 +553,39 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
         const int flags = d.flags;
         if (flags & kFlagTerm) break;
         if (flags & kFlagBegin) {
-            const uint32_t np = d.np;
-            const int ng = (int)((np + (uint32_t)kGroup - 1u) / (uint32_t)kGroup), nsplit = kConsumerWarps / ng, q = warp / ng;
+            const uint32_t nv = d.nv;
+            const int ng = (int)((nv + (uint32_t)kGroup - 1u) / (uint32_t)kGroup), nsplit = kConsumerWarps / ng, q = warp / ng;
             sp = (uint32_t)nsplit | ((uint32_t)ng << 8) | ((uint32_t)q << 16) | ((uint32_t)q << 24);   // first stage of warp q: stage q
             const uint32_t kk = (uint32_t)((warp - q * ng) * kGroup + 2 * lane);
             warp_on = q < nsplit;
-            const bool act = warp_on && kk < np;
+            const bool act = warp_on && kk < nv;
 #pragma unroll
             for (int c = 0; c < (DENS ? 8 : 6); c++) acc64[c][lane] = 0.0;
             nreal = 0;
             if (warp_on) {
                 // lanes past the end of a ragged window shadow its last pair (same pieces, nothing written)
-                const uint32_t p = d.p0 + (act ? kk : np - 2u);
-                const uint32_t *pof = a.poff + d.colbase;
+                const uint32_t v = d.v0 + (act ? kk : nv - 2u);
+                const uint32_t *vof = a.voff + d.colbase;
                 int lo = (int)d.z0, hi = (int)d.z1;
-                while (lo < hi) {                      // last cell of [z0, z1] whose first padded slot is <= p
+                while (lo < hi) {                      // last cell of [z0, z1] whose first sink slot is <= v
                     const int mid = (lo + hi + 1) >> 1;
-                    if (__ldg(pof + mid) <= p) lo = mid; else hi = mid - 1;
+                    if (__ldg(vof + mid) <= v) lo = mid; else hi = mid - 1;
                 }
                 zrel = lo - (int)d.z0;
                 zoff = zrel % nsteps;
                 cell = d.colbase + (uint32_t)lo;
+                const uint32_t r = v - __ldg(vof + lo);                                   // even: the pair (r, r + 1) of the cell
                 const uint32_t o0 = __ldg(a.offset + cell), o1 = __ldg(a.offset + cell + 1);
-                slot = o0 + (p - __ldg(pof + lo));
-                if (act) nreal = slot + 1u < o1 ? 2u : (slot < o1 ? 1u : 0u);
+                const uint32_t p = __ldg(a.poff + cell) + r;                              // its place in the padded source arrays
+                slot = o0 + r;                                                            // r < count: the first of the pair is a particle
+                if (act) nreal = slot + 1u < o1 ? 2u : 1u;
                 const float2 X2 = __ldg(reinterpret_cast<const float2 *>(a.x + p));      // p is even: 8-byte aligned
                 const float2 Y2 = __ldg(reinterpret_cast<const float2 *>(a.y + p));
                 const float2 Z2 = __ldg(reinterpret_cast<const float2 *>(a.z + p));
                 xi = X2; yi = Y2; zi = Z2;
-                // a pad slot next to a real sink takes the real sink's coordinates: it then computes the same (unwritten)
-                // sums and never widens the gap tests below (a pad sits at 2^55)
-                if (slot < o1 && slot + 1u >= o1) { xi.y = xi.x; yi.y = yi.x; zi.y = zi.x; }
+                // the pad slot after the last particle of a cell with an odd count takes that particle's coordinates: it then
+                // computes the same (unwritten) sums and never widens the gap tests below (a pad sits at 2^55)
+                if (slot + 1u >= o1) { xi.y = xi.x; yi.y = yi.x; zi.y = zi.x; }
                 oczs = (double)(float)((double)lo * a.k.cell_w) * a.k.scale;
             }
         }
@@ -628,7 +648,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                         const int q = it < cnt ? qlo + it : kTile / 4;
                         const float dzc = (float)(qz[q] - oczs);
                         const float2 nz = make_float2(dzc - zi.x, dzc - zi.y);
-                        quad<PACKED, MODE, MASS>(sbase[q], py0[q], pz0[q], MASS ? pm0[q] : one, nx, ny, nz, coef, f);
+                        quad<PACKED, MODE, MASS, MODE == 2 && NF_DENS_QV>(sbase[q], py0[q], pz0[q], MASS ? pm0[q] : one, nx, ny, nz, coef, f);
                     }
                 };
                 if (DENS && dens) body(std::integral_constant<int, 2>());
@@ -668,7 +688,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                     if (soft_mode == 1) soft = __any_sync(kFull, touching && gap2 < a.k.soft_thr2);
                     if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
-                if (DENS && dens) piece_loop<PACKED, 2, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                if (DENS && dens) piece_loop<PACKED, 2, MASS, NF_DENS_QV>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
                 else if (soft)    piece_loop<PACKED, 1, MASS, QV>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
                 else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
                 // The FP32 chain of a sink runs over ONE source cell (one step), then joins the FP64 sums: on inputs whose
@@ -788,7 +808,7 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     AccelArgs a;
     a.k = p->k;
     a.x = p->ws.x; a.y = p->ws.y; a.z = p->ws.z; a.m = mass ? p->mass_soa : nullptr;
-    a.poff = p->ws.poff; a.offset = p->ws.offset; a.perm = p->perm;
+    a.poff = p->ws.poff; a.voff = p->ws.voff; a.offset = p->ws.offset; a.perm = p->perm;
     a.units = p->heavy_first ? p->ws.units_sorted : p->ws.units;
     a.n_units = (uint32_t)p->n_units;
     a.counter = &p->ws.scalars[1];

@@ -69,11 +69,12 @@ inline void sort_plan(unsigned long long nkeys, int *passes, int *digit_bits)
     *passes = np; *digit_bits = b;
 }
 
-struct Unit {            // one work unit: a window of <= kChunk consecutive PADDED slots of one z-column (the cells are padded
-                         // to multiples of 4 slots, so an aligned pair of slots never straddles two cells; pad slots are idle sinks)
-    uint32_t p0;         // first padded slot (index into the source arrays x, y, z), a multiple of 4
+struct Unit {            // one work unit: a window of <= kChunk consecutive SINK slots of one z-column.  Sink slots number the
+                         // particles of a column with every cell rounded up to an EVEN count (voff): a lane of the direct kernel
+                         // holds an aligned pair of them, which never straddles two cells; the odd cell's last slot is an idle sink
+    uint32_t v0;         // first sink slot (index into the voff numbering), even
     uint32_t col;        // column id cx * cpd + cy
-    uint16_t np;         // padded slots in the window, a multiple of 4
+    uint16_t nv;         // sink slots in the window, even
     uint16_t z0, z1;     // first and last cell (z index) that hold a slot of the window
     uint16_t flat;       // 1: sparse window (few slots per cell): the direct kernel walks a lane's stencil run in one flat loop
 };
@@ -82,6 +83,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
     uint32_t *cid, *keyA, *keyB, *valA, *valB;   // [n]
     uint32_t *radix_hist;                         // [bins * sort_blocks], digit-major
     uint32_t *count, *offset, *poff, *ubase;      // [C], [C+1], [C+1], [cpd^2+1] (unit base per column)
+    uint32_t *voff;                               // [C+1] sink-slot offsets: exclusive scan of the counts rounded up to even
     uint32_t *src;                                // [C] particles in the stencil of each cell
     uint32_t *scan_tmp;                           // block sums
     float *x, *y, *z;                             // [P_max]

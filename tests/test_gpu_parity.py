@@ -779,7 +779,9 @@ def test_masses_fused_passes_and_errors(oracle_mod):
         a = p.accel().cpu()
         assert_parity(a.numpy().astype(np.float64), ref, "masses with test particles")
         a2, rho = p.accel_density(b)
-        assert torch.equal(a2.cpu(), a) and torch.equal(rho.cpu(), rho_unit)
+        # the fused density pass votes on max(eps_s, b) per four sources, the force-only pass on eps_s: a pair within 0.1 % of
+        # eps_s may or may not take the spline's min (equal there to 1e-7), so the forces agree to rounding, not bit for bit
+        assert ((a2.cpu() - a).norm(dim=1) <= 2e-6 * a.norm(dim=1)).all() and torch.equal(rho.cpu(), rho_unit)
         vel = torch.zeros((cfg.n, 3), device="cuda")
         a3, _ = p.accel_kick(vel, 0.5)
         assert torch.equal(a3.cpu(), a)

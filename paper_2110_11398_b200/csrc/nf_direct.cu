@@ -57,8 +57,15 @@ struct __align__(16) StageDesc {
     uint32_t colbase;          //       col * cpd
     int      oxy;              // column offset: (ox + 128) | (oy + 128) << 8
     int      flat;             // unit flag: sparse window, flat loop
+    // lean stage (flat units whose whole z-run of a neighbour column fits the stage): no piece table; the stage carries the raw
+    // padded offsets of the run's cells (ps[], bulk-copied like the coordinates) in up to three segments -- cells below the
+    // periodic face, inside the box, above it -- and every consumer derives slots and z corners from them
+    int      lean;
+    struct Seg { int ncell, slot0, ps0, jw0; double wz; } seg[3];   // cells, first stage slot, index of the first cell's offset in ps[], wrapped z of the first cell, box wrap
     Piece    pieces[kMaxPieces];
 };
+constexpr int kLeanCells = 256;                 // longest z-run (cells) a lean stage describes
+constexpr int kPsMax = kLeanCells + 3 * 8;      // + alignment slack of the three slices (each starts 16-byte aligned in global memory)
 
 // Pipeline depth: 5 stages for the three coordinate arrays (the consumer warps of a split unit work on different
 // stages at the same time: config 1 0.157 -> 0.137 ms against 3 stages, the large configs unchanged); the mass kernels
@@ -73,6 +80,7 @@ struct __align__(128) SharedStorageT {
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
     double quadz[kStages][kTile / 4 + 1];   // flat loop: z corner (scaled, with box wrap) of the cell of every quad of the stage
+    __align__(16) uint32_t ps[kStages][kPsMax];   // lean stages: padded offsets (poff) of the cells of the run, as copied
     double acc[kConsumerWarps][8][32];    // FP64 sums of every warp's sinks (x, y, z of sink A, x, y, z of sink B, rho A, rho B): kept here, not in
                                           // 16 registers per lane; the warps of a split unit add theirs up from here at the end of the unit
 };
@@ -378,14 +386,16 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
         }
         cp_n = 0;
     };
+    uint32_t extra_tx = 0;                        // bytes of the offset slices of a lean stage
     auto commit = [&](int extra) {
         flush_copy();
         __syncwarp();          // the table entries written by the other lanes are ordered before lane 0's releasing arrive
         if (lead) {
             sm.desc[stage].flags = sflags | extra;
             sm.desc[stage].npieces = np;
-            mbar_arrive_expect_tx(&sm.full[stage], (uint32_t)fill * (4u * NARR));
+            mbar_arrive_expect_tx(&sm.full[stage], (uint32_t)fill * (4u * NARR) + extra_tx);
         }
+        extra_tx = 0;
         if (++stage == kStages) { stage = 0; phase ^= 1u; }
         open = false; sealed = false;
     };
@@ -410,6 +420,67 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                 const float Dy = (float)(((double)(float)((double)jy * k.cell_w) + wy - ocy) * k.scale);
                 const uint32_t row = ((uint32_t)jx * cpd + jy) * cpd;
                 const int soft_mode = k.plummer ? 0 : !(k.fast_ok && a.fastpath) ? 2 : ((ox >= -1 && ox <= 1 && oy >= -1 && oy <= 1) ? 1 : 0);
+                // Lean stage.  In a sparse window (flat unit) the per-cell table below costs the producer ~300 instructions per
+                // 32 cells, one warp against eight: at 4-8 particles per cell the consumers waited for it 15-27 % of the time.
+                // When the whole run of this column fits one stage the producer only reads the offsets at the ends of its (up
+                // to three) segments, copies the coordinates and the offsets themselves, and the consumers do the rest.
+                if (un.flat && jhi - jlo + 1 <= kLeanCells) {
+                    const int sa[3] = {jlo, max(jlo, 0), max(jlo, cpd)}, sb[3] = {min(jhi, -1), min(jhi, cpd - 1), jhi};
+                    const int sh[3] = {cpd, 0, -cpd};
+                    uint32_t v = 0;
+                    {   // lanes 0..5 read the offsets at the two ends of the three segments (selects, no indexed local arrays)
+                        const int q = lane >> 1;
+                        const int qa = q == 0 ? sa[0] : (q == 1 ? sa[1] : sa[2]), qb = q == 0 ? sb[0] : (q == 1 ? sb[1] : sb[2]);
+                        const int qs = q == 0 ? sh[0] : (q == 1 ? sh[1] : sh[2]);
+                        if (lane < 6 && qa <= qb) v = __ldg(a.poff + row + (uint32_t)((lane & 1 ? qb + 1 : qa) + qs));
+                    }
+                    uint32_t g0[3], len[3];
+#pragma unroll
+                    for (int q = 0; q < 3; q++) {
+                        g0[q] = __shfl_sync(kFull, v, 2 * q);
+                        len[q] = __shfl_sync(kFull, v, 2 * q + 1) - g0[q];
+                    }
+                    const uint32_t total = len[0] + len[1] + len[2];
+                    if (total == 0) continue;                     // an empty run never opens a stage
+                    if (total <= (uint32_t)kTile) {
+                        if (open) commit(0);
+                        mbar_wait(&sm.empty[stage], phase ^ 1u);
+                        open = true; sealed = true; fill = (int)total; np = jhi - jlo + 1;
+                        sflags = first ? kFlagBegin : 0;
+                        first = false;
+                        if (lead) {
+                            StageDesc &d = sm.desc[stage];
+                            d.j0 = 0; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
+                            d.v0 = un.v0; d.nv = un.nv; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
+                            d.colbase = un.col * (uint32_t)cpd;
+                            d.lean = 1;
+                            uint32_t slot = 0, psb = 0;
+#pragma unroll
+                            for (int q = 0; q < 3; q++) {
+                                const int nc = sa[q] <= sb[q] ? sb[q] - sa[q] + 1 : 0;
+                                d.seg[q].ncell = nc; d.seg[q].slot0 = (int)slot; d.seg[q].jw0 = sa[q] + sh[q];
+                                d.seg[q].wz = q == 0 ? -k.L : (q == 2 ? k.L : 0.0);
+                                d.seg[q].ps0 = 0;
+                                if (nc > 0) {
+                                    const uint32_t e0 = row + (uint32_t)(sa[q] + sh[q]), al = e0 & ~3u;      // aligned superset of [e0, e0 + nc]
+                                    const uint32_t cnt = (e0 + (uint32_t)nc + 1u - al + 3u) & ~3u;
+                                    d.seg[q].ps0 = (int)(psb + (e0 - al));
+                                    tma_load_1d(&sm.ps[stage][psb], a.poff + al, cnt * 4u, &sm.full[stage]);
+                                    extra_tx += cnt * 4u;
+                                    psb += cnt;
+                                    if (len[q]) {
+                                        tma_load_1d(&sm.buf[stage][0][slot], a.x + g0[q], len[q] * 4u, &sm.full[stage]);
+                                        tma_load_1d(&sm.buf[stage][1][slot], a.y + g0[q], len[q] * 4u, &sm.full[stage]);
+                                        tma_load_1d(&sm.buf[stage][2][slot], a.z + g0[q], len[q] * 4u, &sm.full[stage]);
+                                        if (NARR == 4) tma_load_1d(&sm.buf[stage][NARR - 1][slot], a.m + g0[q], len[q] * 4u, &sm.full[stage]);
+                                    }
+                                    slot += len[q];
+                                }
+                            }
+                        }
+                        continue;
+                    }
+                }
                 for (int jb = jlo; jb <= jhi; jb += 32) {
                     // the warp fetches the padded offsets of up to 32 cells of the run at once
                     const int jl = jb + lane;
@@ -444,6 +515,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 first = false;
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
+                                    d.lean = 0;
                                     d.j0 = jb - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
                                     d.v0 = un.v0; d.nv = un.nv; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
@@ -491,6 +563,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                 first = false;
                                 if (lead) {
                                     StageDesc &d = sm.desc[stage];
+                                    d.lean = 0;
                                     d.j0 = j - jlo; d.soft_mode = soft_mode; d.dx = Dx; d.dy = Dy; d.oxy = (ox + 128) | ((oy + 128) << 8);
                                     d.v0 = un.v0; d.nv = un.nv; d.flat = un.flat; d.z0 = (uint32_t)z0; d.z1 = (uint32_t)z1;
                                     d.colbase = un.col * (uint32_t)cpd;
@@ -623,19 +696,44 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 // of different sink cells read different quads (a few shared-memory wavefronts per load, far from a limit
                 // here).  Every consumer warp fills the table of the stages it works on (same values: no ordering needed).
                 double *qz = sm.quadz[stage];
-                for (int i = lane; i < np; i += 32) {
-                    const Piece pc = d.pieces[i];
-                    for (int q = pc.sm_off >> 2, qe = (pc.sm_off + pc.nslots) >> 2; q < qe; q++) qz[q] = pc.czs;
+                const int ilo = max(ibase, 0), ihi = min(ibase + 2 * R, np - 1);
+                int qlo = 0, cnt = 0;
+                if (d.lean) {
+                    // cell i of the run: its segment, its slots from the copied offsets, its z corner by the producer's formula
+                    const uint32_t *ps = sm.ps[stage];
+                    const int n0 = d.seg[0].ncell, n01 = n0 + d.seg[1].ncell;
+                    auto cell = [&](const int i, int &slot, int &nsl, double &czs) {
+                        const int q = i < n0 ? 0 : (i < n01 ? 1 : 2), li = i - (q == 0 ? 0 : (q == 1 ? n0 : n01));
+                        const StageDesc::Seg sg = d.seg[q];
+                        const uint32_t p0 = ps[sg.ps0 + li], p1 = ps[sg.ps0 + li + 1];
+                        slot = sg.slot0 + (int)(p0 - ps[sg.ps0]); nsl = (int)(p1 - p0);
+                        czs = ((double)(float)((double)(sg.jw0 + li) * a.k.cell_w) + sg.wz) * a.k.scale;
+                    };
+                    for (int i = lane; i < np; i += 32) {
+                        int slot, nsl; double czs;
+                        cell(i, slot, nsl, czs);
+                        for (int q = slot >> 2, qe = (slot + nsl) >> 2; q < qe; q++) qz[q] = czs;
+                    }
+                    if (ilo <= ihi) {
+                        int s0, n0s, s1, n1s; double c0;
+                        cell(ilo, s0, n0s, c0);
+                        cell(ihi, s1, n1s, c0);
+                        qlo = s0 >> 2;
+                        cnt = ((s1 + n1s) >> 2) - qlo;
+                    }
+                } else {
+                    for (int i = lane; i < np; i += 32) {
+                        const Piece pc = d.pieces[i];
+                        for (int q = pc.sm_off >> 2, qe = (pc.sm_off + pc.nslots) >> 2; q < qe; q++) qz[q] = pc.czs;
+                    }
+                    if (ilo <= ihi) {
+                        const Piece pl = d.pieces[ilo], ph = d.pieces[ihi];
+                        qlo = pl.sm_off >> 2;
+                        cnt = ((ph.sm_off + ph.nslots) >> 2) - qlo;
+                    }
                 }
                 if (lane == 0) qz[kTile / 4] = oczs;                 // the dummy quad: any finite corner
                 __syncwarp();
-                const int ilo = max(ibase, 0), ihi = min(ibase + 2 * R, np - 1);
-                int qlo = 0, cnt = 0;
-                if (ilo <= ihi) {
-                    const Piece pl = d.pieces[ilo], ph = d.pieces[ihi];
-                    qlo = pl.sm_off >> 2;
-                    cnt = ((ph.sm_off + ph.nslots) >> 2) - qlo;
-                }
                 const int cmax = __reduce_max_sync(kFull, cnt);
                 const bool soft = soft_mode == 2 || soft_mode == 1;     // near column: the vote decides per quad pair
                 const bool dens = DENS && (a.dens_mode == 2 || gap_dens);

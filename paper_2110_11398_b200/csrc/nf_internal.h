@@ -33,7 +33,10 @@ constexpr int kChunk         = kGroup * kConsumerWarps;   // max sink slots per 
 constexpr int kTile          = NF_TILE;           // source slots per pipeline stage (multiple of 4)
 constexpr int kStages        = NF_STAGES;         // TMA pipeline depth (three staged arrays)
 constexpr int kStagesMass    = NF_STAGES_MASS;    //   with the fourth array of the mass kernels
-constexpr int kMaxPieces     = 40;                // source cells (table entries) per stage
+#ifndef NF_MAX_PIECES
+#define NF_MAX_PIECES 40
+#endif
+constexpr int kMaxPieces     = NF_MAX_PIECES;     // source cells (table entries) per stage
 #ifndef NF_QUAD_VOTE_ABOVE
 #define NF_QUAD_VOTE_ABOVE 4096
 #endif

@@ -697,6 +697,9 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 // here).  Every consumer warp fills the table of the stages it works on (same values: no ordering needed).
                 double *qz = sm.quadz[stage];
                 const int ilo = max(ibase, 0), ihi = min(ibase + 2 * R, np - 1);
+                // the warp fills the table for the cells ITS lanes walk (the runs of 64 consecutive sink slots: a dozen cells), not for
+                // the whole stage; the warps write the same values where their ranges overlap
+                const int wlo = __reduce_min_sync(kFull, ilo <= ihi ? ilo : 0x7fffffff), whi = __reduce_max_sync(kFull, ilo <= ihi ? ihi : -1);
                 int qlo = 0, cnt = 0;
                 if (d.lean) {
                     // cell i of the run: its segment, its slots from the copied offsets, its z corner by the producer's formula
@@ -709,7 +712,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                         slot = sg.slot0 + (int)(p0 - ps[sg.ps0]); nsl = (int)(p1 - p0);
                         czs = ((double)(float)((double)(sg.jw0 + li) * a.k.cell_w) + sg.wz) * a.k.scale;
                     };
-                    for (int i = lane; i < np; i += 32) {
+                    for (int i = wlo + lane; i <= whi; i += 32) {
                         int slot, nsl; double czs;
                         cell(i, slot, nsl, czs);
                         for (int q = slot >> 2, qe = (slot + nsl) >> 2; q < qe; q++) qz[q] = czs;
@@ -722,7 +725,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                         cnt = ((s1 + n1s) >> 2) - qlo;
                     }
                 } else {
-                    for (int i = lane; i < np; i += 32) {
+                    for (int i = wlo + lane; i <= whi; i += 32) {
                         const Piece pc = d.pieces[i];
                         for (int q = pc.sm_off >> 2, qe = (pc.sm_off + pc.nslots) >> 2; q < qe; q++) qz[q] = pc.czs;
                     }
@@ -735,8 +738,10 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 if (lane == 0) qz[kTile / 4] = oczs;                 // the dummy quad: any finite corner
                 __syncwarp();
                 const int cmax = __reduce_max_sync(kFull, cnt);
-                const bool soft = soft_mode == 2 || soft_mode == 1;     // near column: the vote decides per quad pair
-                const bool dens = DENS && (a.dens_mode == 2 || gap_dens);
+                // near column: the spline-capable body (a vote per quad pair) only if some sink of the warp is within eps_s of the
+                // column in x and y (the z gap is not looked at here: conservative); the corner columns almost never are
+                const bool soft = soft_mode == 2 || (soft_mode == 1 && __any_sync(kFull, gxy2 < a.k.soft_thr2));
+                const bool dens = DENS && (a.dens_mode == 2 || (gap_dens && __any_sync(kFull, gxy2 < a.dens_thr2)));
                 const float4 *py0 = sbase + kTileAlloc / 4, *pz0 = py0 + kTileAlloc / 4, *pm0 = pz0 + kTileAlloc / 4;
                 const float4 one = make_float4(1.f, 1.f, 1.f, 1.f);
                 auto body = [&](auto mode) {

@@ -699,7 +699,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 const int ilo = max(ibase, 0), ihi = min(ibase + 2 * R, np - 1);
                 // the warp fills the table for the cells ITS lanes walk (the runs of 64 consecutive sink slots: a dozen cells), not for
                 // the whole stage; the warps write the same values where their ranges overlap
-                const int wlo = __reduce_min_sync(kFull, ilo <= ihi ? ilo : 0x7fffffff), whi = __reduce_max_sync(kFull, ilo <= ihi ? ihi : -1);
+                const int wlo = __reduce_min_sync(kFull, ilo <= ihi ? ilo : np), whi = __reduce_max_sync(kFull, ilo <= ihi ? ihi : -1);   // none: [np, -1] is empty
                 int qlo = 0, cnt = 0;
                 if (d.lean) {
                     // cell i of the run: its segment, its slots from the copied offsets, its z corner by the producer's formula

@@ -42,7 +42,7 @@ constexpr int kMaxPieces     = NF_MAX_PIECES;     // source cells (table entries
 #endif
 constexpr unsigned kQuadVoteAbove = NF_QUAD_VOTE_ABOVE;   // fullest cell above this: launch the quad-vote instance of the direct kernel
 #ifndef NF_FLAT_BELOW
-#define NF_FLAT_BELOW 14
+#define NF_FLAT_BELOW 22
 #endif
 constexpr int kFlatBelow     = NF_FLAT_BELOW;     // default of the "flat_below" option (padded slots per spanned cell)
 constexpr int kAccelThreads  = 32 * (kConsumerWarps + 1);   // + 1 producer warp

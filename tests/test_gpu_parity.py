@@ -1014,8 +1014,8 @@ def test_rebin_full_size(oracle_mod, idx, device):
 
 
 # ---------------------------------------------------------------- sparse windows: the flat loop of the direct kernel
-@pytest.mark.parametrize("n,cpd,R,flat_below", [(8000, 10, 2, 14), (8000, 16, 2, 14), (6000, 20, 2, 14), (8000, 16, 2, 0), (20000, 12, 3, 1024),
-                                                (30000, 9, 2, 1024), (3000, 25, 1, 14)])
+@pytest.mark.parametrize("n,cpd,R,flat_below", [(8000, 10, 2, 22), (8000, 16, 2, 22), (6000, 20, 2, 22), (8000, 16, 2, 0), (20000, 12, 3, 1024),
+                                                (30000, 9, 2, 1024), (3000, 25, 1, 22), (8000, 16, 2, 14)])
 def test_sparse_flat_loop(oracle_mod, n, cpd, R, flat_below):
     """Windows with a handful of slots per cell walk a lane's stencil run in one flat loop (nf_set_option "flat_below"):
     8, 2 and 0.75 particles per cell with the default threshold, the same grid with the flat loop switched off, and dense
@@ -1034,3 +1034,42 @@ def test_sparse_flat_loop(oracle_mod, n, cpd, R, flat_below):
         ref_rho = oracle_mod.density(pos.numpy(), cpd, 1.0, 0.4 / cpd, R)
         assert (np.abs(rho.cpu().numpy().astype(np.float64) - ref_rho) / ref_rho).max() <= 1e-5
         assert (acc.cpu().double().numpy() - out["acc"]).__abs__().max() <= 1e-5 * np.abs(out["acc"]).max()
+
+
+@pytest.mark.parametrize("kind,n,cpd,R,flat_below", [
+    ("uniform", 20000, 5, 2, 1024),      # cpd = 2R+1, one window spans the column: the run [-2, 6] has THREE periodic segments
+    ("uniform", 2500, 7, 3, 1024),       # the same with R = 3 (run longer than the column)
+    ("uniform", 60000, 6, 2, 1024),      # forced flat on dense cells: the run exceeds a stage, the producer falls back to the piece table
+    ("columns", 3000, 300, 2, 22),       # ten columns of a 300^3 grid: one window spans 300 cells, above the 256 a lean stage describes
+    ("columns", 2000, 250, 2, 22),       # 254-cell runs: the longest a lean stage takes, through both periodic faces
+    ("faces", 6000, 24, 2, 22),          # particles crowded at z = 0 and z = L: every run of the face windows wraps
+])
+def test_lean_stages(oracle_mod, kind, n, cpd, R, flat_below):
+    """Lean stages of the flat loop: the producer copies the padded offsets of a whole z-run instead of building
+    a per-cell table.  Runs in one, two and three periodic segments, the two fallbacks to the piece table (more slots than a
+    stage, more cells than a lean stage describes) and a mix of both in one unit -- each against the oracle, and against the
+    stepped loop of the same binning (flat_below = 0; the FP32 chains are cut at different places, so not bit for bit)."""
+    g = torch.Generator().manual_seed(7 * n + cpd)
+    pos = torch.rand((n, 3), generator=g)
+    if kind == "columns":
+        cols = torch.randint(0, cpd, (10, 2), generator=g).float()
+        pick = torch.randint(0, 10, (n,), generator=g)
+        pos[:, 0] = (cols[pick, 0] + pos[:, 0]) / cpd
+        pos[:, 1] = (cols[pick, 1] + pos[:, 1]) / cpd
+    elif kind == "faces":
+        pos[: n // 2, 2] = torch.remainder(0.02 * torch.randn(n // 2, generator=g), 1.0)
+    pos = torch.remainder(pos, 1.0).to(torch.float32).contiguous()
+    pos[pos >= 1.0] = 0.0
+    eps = 0.01 / cpd
+    st, out = full_check(oracle_mod, pos, cpd, 1.0, eps, R, options={"flat_below": flat_below}, what=f"lean {kind} n={n} cpd={cpd} R={R}")
+    import paper_2110_11398_b200 as nf
+    res = []
+    for fb in (flat_below, 0):
+        with nf.Plan(cpd, 1.0, eps, R) as plan:
+            plan.set_option("flat_below", fb)
+            plan.bin(pos.cuda())
+            res.append(plan.accel().cpu().numpy())
+    d = np.abs(res[0].astype(np.float64) - res[1]).max(axis=1)
+    scale = np.abs(out["acc"]).max(axis=1) + 1e-300
+    # both are within 1e-5 (99.9 %) / 1e-3 of the oracle; against each other the triangle inequality gives twice that
+    assert np.quantile(d / scale, 0.999) <= 2e-5 and (d / scale).max() <= 2e-3, (np.quantile(d / scale, 0.999), (d / scale).max())

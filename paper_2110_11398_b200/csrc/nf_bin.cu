@@ -549,9 +549,12 @@ __global__ void __launch_bounds__(256) colunits_kernel(Consts k, const uint32_t 
 }
 
 // One thread per column walks its cells once and emits the column's units with their cost keys.
+// The sort key of a unit: clz of its interaction count (heavier -> smaller key, 0..64) with the flat flag above it, so that
+// the one stable radix pass on the key also puts the flat units (sparse windows) behind all the others: nf_accel then runs
+// the stepped units and the flat units as two launches of two kernel instances, each holding one loop structure only.
 __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__restrict__ voff, const uint32_t *__restrict__ count,
                                                     const uint32_t *__restrict__ src, const uint32_t *__restrict__ ubase,
-                                                    Unit *__restrict__ units, uint32_t *__restrict__ ukey)
+                                                    Unit *__restrict__ units, uint32_t *__restrict__ ukey, uint32_t *__restrict__ n_flat)
 {
     const uint32_t col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= (uint32_t)(k.cpd * k.cpd)) return;
@@ -561,7 +564,7 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
     int rel = (int)(col / (uint32_t)k.cpd) - k.slab0; rel += rel < 0 ? k.cpd : 0;
     if (rel >= k.nslab) return;
     const uint32_t c_begin = off[0], c_end = off[k.cpd];
-    uint32_t u = ubase[col];
+    uint32_t u = ubase[col], nflat = 0;
     int z = 0;
     for (uint32_t s0 = c_begin, len = 0; s0 < c_end; s0 += len, u++) {
         len = window_len(c_end - s0, (uint32_t)k.chunk);
@@ -578,11 +581,15 @@ __global__ void __launch_bounds__(128) units_kernel(Consts k, const uint32_t *__
             zz++;
         }
         un.z1 = (uint16_t)zz;
-        un.flat = (uint16_t)((uint32_t)un.nv < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
+        // sparse: the cells the window touches hold few slots on average (all their slots, not the part inside the window: the
+        // short last window of a dense column is not sparse)
+        un.flat = (uint16_t)(off[zz + 1] - off[z] < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
         units[u] = un;
-        ukey[u] = (uint32_t)__clzll((long long)cost);     // heavier -> smaller key
+        ukey[u] = (uint32_t)__clzll((long long)cost) | ((uint32_t)un.flat << 7);     // heavier -> smaller key; flat units last
+        nflat += un.flat;
         z = zz;
     }
+    if (nflat) atomicAdd(n_flat, nflat);
 }
 
 __global__ void __launch_bounds__(256) units_permute_kernel(const Unit *__restrict__ in, const uint32_t *__restrict__ order,
@@ -704,7 +711,9 @@ __global__ void __launch_bounds__(1024) small_units_kernel(Consts k, const uint3
                 zz++;
             }
             un.z1 = (uint16_t)zz;
-            un.flat = (uint16_t)((uint32_t)un.nv < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
+            // sparse: the cells the window touches hold few slots on average (all their slots, not the part inside the window: the
+        // short last window of a dense column is not sparse)
+        un.flat = (uint16_t)(off[zz + 1] - off[z] < (uint32_t)k.flat_below * (uint32_t)(zz - z + 1) ? 1 : 0);
             units[u] = un;
             const uint32_t key = (uint32_t)__clzll((long long)cost);
             s_key[u] = (unsigned char)key;
@@ -752,7 +761,7 @@ static int launch_units(nf_plan *p, size_t n, uint32_t *free_key, uint32_t *free
     cellcost_kernel<<<nbc, 256, 0, st>>>(k, ws.count, ws.src, ws.interactions, &ws.scalars[7]);  L++;
     colunits_kernel<<<(ncols + 255) / 256, 256, 0, st>>>(k, ws.voff, ws.ubase);  L++;
     exclusive_scan(ws.ubase, ws.ubase, (size_t)ncols, ws.scan_tmp, OpId(), 1, &ws.scalars[2], st, &L);
-    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.voff, ws.count, ws.src, ws.ubase, ws.units, ukey);  L++;
+    units_kernel<<<(ncols + 127) / 128, 128, 0, st>>>(k, ws.voff, ws.count, ws.src, ws.ubase, ws.units, ukey, &ws.scalars[8]);  L++;
     NF_CUDA_OK(cudaGetLastError());
 
     // heavy-first order: the unit count stays on the device (scalars[2]); the sort's grids cover the host-side bound
@@ -846,12 +855,13 @@ int launch_bin(nf_plan *p, const float *pos, long long n_ll)
     NF_CUDA_OK(cudaGetLastError());
     // domain flag + unit count: the one documented synchronisation of nf_bin, at the END of the call -- nothing is
     // enqueued after it, so the binning is complete on return whatever stream the caller uses next
-    uint32_t sc[8];
+    uint32_t sc[16];
     NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));
     NF_CUDA_OK(cudaStreamSynchronize(st));
     if (sc[0]) { set_error("nf_bin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
     p->n_units = (long long)sc[2];
     p->max_count = sc[7];
+    p->n_flat = small || !p->heavy_first ? -1 : (long long)sc[8];   // -1: the unit list is not partitioned (flat units anywhere)
     p->have_bin_time = true;
     p->launches_bin = L;
     return NF_OK;
@@ -1206,7 +1216,7 @@ int launch_rebin(nf_plan *p, const float *pos)
     { const int rc = launch_units(p, n, const_cast<uint32_t *>(slotcell_old), const_cast<uint32_t *>(perm_old), &L); if (rc != NF_OK) return rc; }
     NF_CUDA_OK(cudaEventRecord(p->ev[1], st));
     NF_CUDA_OK(cudaGetLastError());
-    uint32_t sc[8];
+    uint32_t sc[16];
     NF_CUDA_OK(cudaMemcpyAsync(sc, ws.scalars, sizeof(sc), cudaMemcpyDeviceToHost, st));   // the call's one synchronisation, at its end
     NF_CUDA_OK(cudaStreamSynchronize(st));
     if (sc[0]) { set_error("nf_rebin: a coordinate is non-finite or outside [0, L)"); return NF_ERR_DOMAIN; }
@@ -1218,6 +1228,7 @@ int launch_rebin(nf_plan *p, const float *pos)
     p->rebin_path = 1;
     p->n_units = (long long)sc[2];
     p->max_count = sc[7];
+    p->n_flat = !p->heavy_first ? -1 : (long long)sc[8];
     p->have_bin_time = true;
     p->launches_bin = L;
     return NF_OK;

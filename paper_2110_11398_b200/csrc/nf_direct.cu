@@ -72,15 +72,15 @@ constexpr int kPsMax = kLeanCells + 3 * 8;      // + alignment slack of the thre
 // stage a fourth array and keep 3 so that three CTAs still fit an SM.
 template <int NARR> struct StagesFor { static constexpr int value = NARR == 3 ? kStages : kStagesMass; };
 
-template <int NARR>                    // 3: x, y, z;  4: + the source masses (nf_set_masses)
+template <int NARR, bool FLAT = true>  // NARR 3: x, y, z;  4: + the source masses (nf_set_masses).  FLAT = false: no flat loop, no tables for it
 struct __align__(128) SharedStorageT {
     static constexpr int kStages = StagesFor<NARR>::value;
     float buf[kStages][NARR][kTile + 4];  // x, y, z (, m) of the staged sources + one quad of dummies (never overwritten)
     StageDesc desc[kStages];
     unsigned long long full[kStages];
     unsigned long long empty[kStages];
-    double quadz[kStages][kTile / 4 + 1];   // flat loop: z corner (scaled, with box wrap) of the cell of every quad of the stage
-    __align__(16) uint32_t ps[kStages][kPsMax];   // lean stages: padded offsets (poff) of the cells of the run, as copied
+    double quadz[FLAT ? kStages : 1][FLAT ? kTile / 4 + 1 : 1];   // flat loop: z corner (scaled, with box wrap) of the cell of every quad of the stage
+    __align__(16) uint32_t ps[FLAT ? kStages : 1][FLAT ? kPsMax : 4];   // lean stages: padded offsets (poff) of the cells of the run, as copied
     double acc[kConsumerWarps][8][32];    // FP64 sums of every warp's sinks (x, y, z of sink A, x, y, z of sink B, rho A, rho B): kept here, not in
                                           // 16 registers per lane; the warps of a split unit add theirs up from here at the end of the unit
 };
@@ -365,8 +365,8 @@ struct AccelArgs {
 
 // The producer warp runs in lockstep (all control flow is warp-uniform); lane 0 alone touches the
 // descriptors, the barriers and the TMA unit.
-template <int NARR>
-__device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR> &sm, const int lane)
+template <int NARR, bool FLAT>
+__device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR, FLAT> &sm, const int lane)
 {
     constexpr int kStages = StagesFor<NARR>::value;
     const Consts &k = a.k;
@@ -424,7 +424,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                 // 32 cells, one warp against eight: at 4-8 particles per cell the consumers waited for it 15-27 % of the time.
                 // When the whole run of this column fits one stage the producer only reads the offsets at the ends of its (up
                 // to three) segments, copies the coordinates and the offsets themselves, and the consumers do the rest.
-                if (un.flat && jhi - jlo + 1 <= kLeanCells) {
+                if (FLAT && un.flat && jhi - jlo + 1 <= kLeanCells) {
                     const int sa[3] = {jlo, max(jlo, 0), max(jlo, cpd)}, sb[3] = {min(jhi, -1), min(jhi, cpd - 1), jhi};
                     const int sh[3] = {cpd, 0, -cpd};
                     uint32_t v = 0;
@@ -594,8 +594,8 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV>
-__device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS ? 4 : 3> &sm, const int warp, const int lane)
+template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV, bool FLAT>
+__device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS ? 4 : 3, FLAT> &sm, const int warp, const int lane)
 {
     const float dens_r2 = DENS ? -1.001f / a.dens_nb2 + a.k.tiny : 0.f;
     const SoftCoef coef = {a.k.A, a.k.B, a.k.C, a.k.tiny, a.k.soft_r2, DENS ? a.dens_nb2 : 0.f, dens_r2, a.k.plummer,
@@ -689,7 +689,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 if (DENS) { acc64[6][lane] += (double)f.rho.x; acc64[7][lane] += (double)f.rho.y; }
                 f.clear();
             };
-            if (d.flat) {
+            if (FLAT && d.flat) {
                 // Sparse window (a handful of slots per cell): a lane's 2R+1 stencil cells of this column are ONE contiguous
                 // run of quads in the stage, walked in one loop with the cell's z corner looked up per quad -- instead of
                 // 2R+1 steps that each pay ~50 instructions of piece lookup and warp reductions for one or two quads.  Lanes
@@ -839,13 +839,18 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
     }
 }
 
-template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV = false>
+// FLAT = false: an instance WITHOUT the flat loop and the lean stages, for the launch that holds no flat unit (nf_bin sorts
+// them behind all the others): the stepped pair loops then keep the registers and uniform registers they had before the
+// sparse path grew (with both in one instance ptxas re-loaded `tiny` and the spline coefficient from the constant bank
+// inside the quad-vote loop: config 4 -1.6 %, config 5 -1.8 %).  A flat unit that reaches such an instance is still
+// computed correctly, by the stepped loop.
+template <bool PACKED, bool DENS, bool EPI, bool MASS, bool QV = false, bool FLAT = true>
 __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(const AccelArgs a)
 {
     constexpr int NARR = MASS ? 4 : 3;
     constexpr int kStages = StagesFor<NARR>::value;
     extern __shared__ __align__(128) unsigned char smem_raw[];          // dynamic: stages above 48 KB need the opt-in
-    SharedStorageT<NARR> &sm = *reinterpret_cast<SharedStorageT<NARR> *>(smem_raw);
+    SharedStorageT<NARR, FLAT> &sm = *reinterpret_cast<SharedStorageT<NARR, FLAT> *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < kStages * NARR * 4)                                       // dummy quad: far-away coordinates, mass 0
         sm.buf[tid / (4 * NARR)][(tid / 4) % NARR][kTile + (tid & 3)] = (tid / 4) % NARR == 3 ? 0.f : kDummy;
@@ -854,8 +859,8 @@ __global__ void __launch_bounds__(kAccelThreads, kMinCtasPerSm) direct_kernel(co
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (warp == kConsumerWarps) producer<NARR>(a, sm, lane);
-    else                        consumer<PACKED, DENS, EPI, MASS, QV>(a, sm, warp, lane);
+    if (warp == kConsumerWarps) producer<NARR, FLAT>(a, sm, lane);
+    else                        consumer<PACKED, DENS, EPI, MASS, QV, FLAT>(a, sm, warp, lane);
 }
 
 typedef void (*direct_fn)(const AccelArgs);
@@ -865,8 +870,13 @@ static direct_fn pick_kernel_m(int variant, bool dens, bool epi)    // dens and 
     if (variant == 0) return dens ? direct_kernel<true, true, false, MASS> : (epi ? direct_kernel<true, false, true, MASS> : direct_kernel<true, false, false, MASS>);
     return dens ? direct_kernel<false, true, false, MASS> : (epi ? direct_kernel<false, false, true, MASS> : direct_kernel<false, false, false, MASS>);
 }
-static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false, bool qv = false)
+static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false, bool qv = false, bool noflat = false)
 {
+    // the instances without the flat loop exist for the packed force-only kernels with unit masses (plain and fused epilogue)
+    if (noflat && variant == 0 && !dens && !mass) {
+        if (qv) return epi ? direct_kernel<true, false, true, false, true, false> : direct_kernel<true, false, false, false, true, false>;
+        return epi ? direct_kernel<true, false, true, false, false, false> : direct_kernel<true, false, false, false, false, false>;
+    }
     // the quad-vote instances exist for the packed force-only kernels (plain and fused epilogue, with and without masses:
     // which pairs next to eps_s see the spline's min depends on the vote granularity, at the level of one ulp of that
     // pair, so the mass kernel must follow the plain one for "all masses 1 = the same bits")
@@ -876,7 +886,11 @@ static direct_fn pick_kernel(int variant, bool dens, bool epi, bool mass = false
     }
     return mass ? pick_kernel_m<true>(variant, dens, epi) : pick_kernel_m<false>(variant, dens, epi);
 }
-static size_t smem_bytes(bool mass) { return mass ? sizeof(SharedStorageT<4>) : sizeof(SharedStorageT<3>); }
+static size_t smem_bytes(bool mass, bool flat = true)
+{
+    if (!flat) return sizeof(SharedStorageT<3, false>);          // the instances without the flat loop are unit-mass kernels
+    return mass ? sizeof(SharedStorageT<4>) : sizeof(SharedStorageT<3>);
+}
 
 int accel_max_ctas_per_sm(int variant)
 {
@@ -898,23 +912,33 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
     if (p->n == 0 || p->n_units == 0) return NF_OK;
     const bool dens = rho != nullptr;
     const bool mass = p->have_mass;
-    const size_t smem = smem_bytes(mass);
     p->quad_vote = p->quad_vote_opt >= 0 ? p->quad_vote_opt : (p->max_count > kQuadVoteAbove ? 1 : 0);
-    direct_fn fn = pick_kernel(p->variant, dens, vel != nullptr || amax_cell != nullptr, mass, p->quad_vote != 0);
-    int per_sm = 0;
-    NF_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kAccelThreads, smem) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
-    if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
-    if (p->ctas_per_sm > 0 && p->ctas_per_sm < per_sm) per_sm = p->ctas_per_sm;
-    long long grid = (long long)p->sm_count * per_sm;
-    if (grid > p->n_units) grid = p->n_units;
+    const bool epi = vel != nullptr || amax_cell != nullptr;
+    // nf_bin sorted the flat units (sparse windows) behind all the others: the stepped units go to an instance without the
+    // flat loop, the flat units to the instance that has it (never the quad-vote one: heavy cells are not flat) -- two
+    // launches, one after the other on the plan's stream.  Where no such instance exists (density, masses, scalar variant) or
+    // the list is not partitioned (small problems, heavy_first = 0) one launch of the instance with both loops does it all.
+    const bool split = p->n_flat >= 0 && p->heavy_first && p->variant == 0 && !dens && !mass;
+    const long long n_step = split ? p->n_units - p->n_flat : p->n_units;
+    direct_fn fns[2] = {pick_kernel(p->variant, dens, epi, mass, p->quad_vote != 0, split), pick_kernel(p->variant, dens, epi, mass, false, false)};
+    long long first[2] = {0, n_step}, count[2] = {n_step, p->n_units - n_step}, grids[2] = {0, 0};
+    const size_t smems[2] = {smem_bytes(mass, !split), smem_bytes(mass, true)};
+    for (int l = 0; l < 2; l++) {
+        if (count[l] <= 0) continue;
+        int per_sm = 0;
+        const size_t smem = smems[l];
+        NF_CUDA_OK(cudaFuncSetAttribute(fns[l], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fns[l], kAccelThreads, smem) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        if (per_sm <= 0) { set_error("direct_kernel cannot be resident on this device (occupancy query returned 0)"); return NF_ERR_CUDA; }
+        if (p->ctas_per_sm > 0 && p->ctas_per_sm < per_sm) per_sm = p->ctas_per_sm;
+        grids[l] = (long long)p->sm_count * per_sm;
+        if (grids[l] > count[l]) grids[l] = count[l];
+    }
     AccelArgs a;
     a.k = p->k;
     a.x = p->ws.x; a.y = p->ws.y; a.z = p->ws.z; a.m = mass ? p->mass_soa : nullptr;
     a.poff = p->ws.poff; a.voff = p->ws.voff; a.offset = p->ws.offset; a.perm = p->perm;
-    a.units = p->heavy_first ? p->ws.units_sorted : p->ws.units;
-    a.n_units = (uint32_t)p->n_units;
-    a.counter = &p->ws.scalars[1];
+    const Unit *units = p->heavy_first ? p->ws.units_sorted : p->ws.units;
     a.acc = acc;
     a.fastpath = p->fastpath;
     a.rho = rho; a.dens_nb2 = 0.f; a.dens_thr2 = 0.f; a.dens_mode = 0;
@@ -927,14 +951,22 @@ int launch_accel(nf_plan *p, float *acc, float *rho, double b, float *vel, doubl
         a.dens_mode = (b <= 0.999 * p->k.cell_w) ? 1 : 2;
     }
     NF_CUDA_OK(cudaEventRecord(p->ev[2], st));
-    NF_CUDA_OK(cudaMemsetAsync(a.counter, 0, 4, st));
+    NF_CUDA_OK(cudaMemsetAsync(&p->ws.scalars[1], 0, 4, st));        // the two work counters (scalars 1 and 9)
+    NF_CUDA_OK(cudaMemsetAsync(&p->ws.scalars[9], 0, 4, st));
     if (amax_cell) NF_CUDA_OK(cudaMemsetAsync(amax_cell, 0, 4 * (size_t)p->k.ncells, st));
-    fn<<<(unsigned)grid, kAccelThreads, smem, st>>>(a);
-    NF_CUDA_OK(cudaGetLastError());
+    p->accel_grid = 0;
+    for (int l = 0; l < 2; l++) {
+        if (count[l] <= 0) continue;
+        a.units = units + first[l];
+        a.n_units = (uint32_t)count[l];
+        a.counter = &p->ws.scalars[l == 0 ? 1 : 9];
+        fns[l]<<<(unsigned)grids[l], kAccelThreads, smems[l], st>>>(a);
+        NF_CUDA_OK(cudaGetLastError());
+        if (grids[l] > p->accel_grid) p->accel_grid = (int)grids[l];
+        p->launches_accel++;
+    }
     NF_CUDA_OK(cudaEventRecord(p->ev[3], st));
     p->have_accel_time = true;
-    p->accel_grid = (int)grid;
-    p->launches_accel = 1;
     return NF_OK;
 }
 

@@ -95,7 +95,8 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
     unsigned long long *interactions;             // [1]
     uint32_t *scalars;                            // [64]: 0 error flag, 1 unit counter, 2 n_units, 3 padded total,
                                                   //       4 movers of the last nf_rebin, 5 rebin fallback flag, 6 look-back ticket,
-                                                  //       7 particles in the fullest cell
+                                                  //       7 particles in the fullest cell, 8 flat units, 9 unit counter of the
+                                                  //       second launch of nf_accel
     // incremental re-binning (nf_rebin)
     uint32_t *offset_new;                         // [C+2]
     uint32_t *arr_count, *arr_off, *arr_cursor;   // [C+2] arrivals per cell, their exclusive scan, fill cursors
@@ -109,7 +110,7 @@ struct Workspace {       // carved out of one arena; all 256-byte aligned
 struct Consts {          // everything the kernels need about the problem, by value
     int cpd, R;
     int chunk;                      // sink slots per work unit (window of one z-column), 64..kChunk
-    int flat_below;                 // windows with fewer padded slots per spanned cell than this take the flat loop (0: none)
+    int flat_below;                 // windows whose cells hold fewer sink slots on average than this take the flat loop (0: none)
     int slab0, nslab;               // sink slabs: cells with x index in {slab0, ..., slab0 + nslab - 1} mod cpd (default: all)
     uint32_t ncells;
     double L, cell_w, inv_cell_w;   // inv_cell_w = cpd / L
@@ -139,6 +140,7 @@ struct nf_plan {
     // state of the last binning
     long long n;  bool binned;
     long long n_units;
+    long long n_flat;               // flat units, sorted behind all the others in units_sorted; -1: the list is not partitioned
     int sort_passes;
     const uint32_t *perm;
     const uint32_t *slotcell;       // cell of every sorted slot (nf_rebin keeps it; NULL after a full nf_bin until first needed)

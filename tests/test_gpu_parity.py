@@ -1073,3 +1073,24 @@ def test_lean_stages(oracle_mod, kind, n, cpd, R, flat_below):
     scale = np.abs(out["acc"]).max(axis=1) + 1e-300
     # both are within 1e-5 (99.9 %) / 1e-3 of the oracle; against each other the triangle inequality gives twice that
     assert np.quantile(d / scale, 0.999) <= 2e-5 and (d / scale).max() <= 2e-3, (np.quantile(d / scale, 0.999), (d / scale).max())
+
+
+def test_flat_units_take_their_own_launch(oracle_mod):
+    """nf_bin sorts the flat units (sparse windows) behind all the others and nf_accel runs the two groups as two launches of
+    two kernel instances.  A box with a dense half and a sparse half: two launches, against the oracle, and bit
+    for bit what ONE launch of the instance that holds both loops gives (heavy_first = 0: the list is not partitioned)."""
+    import paper_2110_11398_b200 as nf
+    g = torch.Generator().manual_seed(31)
+    n, cpd = 60000, 20
+    pos = torch.rand((n, 3), generator=g)
+    pos[: n * 9 // 10, 0] *= 0.5                                  # nine tenths of the particles in the half x < 1/2
+    pos = pos.to(torch.float32).contiguous()
+    st, out = full_check(oracle_mod, pos, cpd, 1.0, 0.01 / cpd, 2, what="dense half + sparse half")
+    assert out["stats"]["kernel_launches_accel"] == 2, out["stats"]
+    one = gpu_run(pos, cpd, 1.0, 0.01 / cpd, 2, options={"heavy_first": 0})
+    assert one["stats"]["kernel_launches_accel"] == 1, one["stats"]
+    assert np.array_equal(one["acc"], out["acc"])
+    # all flat, none flat: one launch each
+    assert gpu_run(pos, cpd, 1.0, 0.01 / cpd, 2, options={"flat_below": 0})["stats"]["kernel_launches_accel"] == 1
+    sparse = torch.rand((4000, 3), generator=g).to(torch.float32)
+    assert gpu_run(sparse, 24, 1.0, 0.01 / 24, 2)["stats"]["kernel_launches_accel"] == 1

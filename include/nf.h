@@ -63,7 +63,7 @@ typedef struct nf_stats {
     int   accel_grid;          /* CTAs of the persistent direct-sum launch */
     int   accel_block;         /* threads per CTA */
     int   kernel_launches_bin; /* kernels launched by one nf_bin */
-    int   kernel_launches_accel; /* kernels launched by one nf_accel */
+    int   kernel_launches_accel; /* kernels launched by one nf_accel: 1, or 2 when the binning holds dense and sparse windows */
     int   rebin_path;          /* last nf_rebin: 1 = incremental merge, 2 = sorted from scratch; 0 = none since nf_bin */
     long long rebin_movers;    /* particles that changed cell in the last incremental nf_rebin (-1: not counted) */
 } nf_stats;
@@ -278,8 +278,9 @@ int nf_get_stats(nf_plan *plan, nf_stats *out);
  *                  again.  With 512-slot windows the remainder of a column is cut into 256 / 128 / fewer slots (sink
  *                  groups that divide the consumer warps).  Accelerations are bit-identical between plans only for equal
  *                  windows.  Takes effect at the next nf_bin.
- *   "flat_below"   windows with fewer padded slots per spanned cell than this walk a lane's stencil run in one flat loop
- *                  (sparse cells: DESIGN.md 7); default 14, 0 = never.  Takes effect at the next nf_bin.
+ *   "flat_below"   windows whose cells hold fewer sink slots on average than this walk a lane's stencil run in one flat loop
+ *                  (sparse cells: DESIGN.md 7); default 22, 0 = never.  Takes effect at the next nf_bin.  nf_bin sorts these
+ *                  windows behind all the others and nf_accel runs them as a second launch (kernel_launches_accel = 2).
  *   "quad_vote"    -1 (default) = the direct-kernel instance that votes once per four sources in the spline-capable loop is
  *                  launched when the fullest cell of the binning holds more than 4096 particles (the halo cells of clustered
  *                  inputs spend nearly all their pairs in that loop); 0 = never, 1 = always.  The two instances agree to one ulp of the

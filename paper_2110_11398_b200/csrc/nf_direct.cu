@@ -162,6 +162,12 @@ constexpr int kUnrollSoft = NF_UNROLL_SOFT;   // unrolling of the spline-capable
 #define NF_UNROLL_TAIL 8
 #endif
 constexpr int kUnrollTail = NF_UNROLL_TAIL;   // unrolling of the ragged tail (whole pieces run there when a lane of the warp has none)
+#ifndef NF_UNROLL_TAIL_QV
+#define NF_UNROLL_TAIL_QV 4
+#endif
+constexpr int kUnrollTailQV = NF_UNROLL_TAIL_QV;   // the same in the quad-vote instances: the choice moves ptxas's register allocation of the
+                                                   // whole kernel, and with 4 the quad-vote loop has 20 same-bank operand pairs instead of 25
+                                                   // (config 4 +0.3 %, config 5 +0.5 %; the other instances lose 0.15 % with it)
 constexpr int kTileAlloc = kTile + 4;          // + one quad of dummies that every lane may read past its piece
 #ifndef NF_DENS_QV
 #define NF_DENS_QV 1                           // fused density loops: one combined vote per quad (1) or two votes per two sources (0)
@@ -311,7 +317,7 @@ __device__ __forceinline__ void quad(const float4 X, const float4 Y, const float
 // in the ragged tail a lane that has run out of sources is predicated off (Newtonian body) or reads the stage's
 // dummy quad (coordinates 2^55: contributes exactly 0 to the force and to the density) so that the warp stays
 // converged for the vote of the spline body.
-template <bool PACKED, int MODE, bool MASS, bool QV = false>
+template <bool PACKED, int MODE, bool MASS, bool QV = false, int UT = kUnrollTail>
 __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const int n4, const int nmin, const int nmax,
                                            const uint32_t live, const int jdummy, const float2 nx, const float2 ny, const float2 nz,
                                            const SoftCoef &c, Partial &f)
@@ -330,7 +336,7 @@ __device__ __forceinline__ void piece_loop(const float4 *__restrict__ px, const 
         }
     }
     __syncwarp();
-#pragma unroll kUnrollTail
+#pragma unroll UT
     for (int j = nmin; j < nmax; j++) {
         if (MODE >= 1) {                              // the body votes: keep the warp converged
             const int jj = j < n4 ? j : jdummy;
@@ -791,9 +797,10 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                     if (soft_mode == 1) soft = __any_sync(kFull, touching && gap2 < a.k.soft_thr2);
                     if (gap_dens) dens = __any_sync(kFull, touching && gap2 < a.dens_thr2);
                 }
-                if (DENS && dens) piece_loop<PACKED, 2, MASS, NF_DENS_QV>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
-                else if (soft)    piece_loop<PACKED, 1, MASS, QV>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
-                else              piece_loop<PACKED, 0, MASS>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                constexpr int UT = QV ? kUnrollTailQV : kUnrollTail;
+                if (DENS && dens) piece_loop<PACKED, 2, MASS, NF_DENS_QV, UT>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                else if (soft)    piece_loop<PACKED, 1, MASS, QV, UT>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
+                else              piece_loop<PACKED, 0, MASS, false, UT>(px, n4, nmin, nmax, live, jdummy, nx, ny, nz, coef, f);
                 // The FP32 chain of a sink runs over ONE source cell (one step), then joins the FP64 sums: on inputs whose
                 // pair forces nearly cancel (config 2, a barely perturbed lattice) the rounding of a chain grows with its
                 // length (error ~ 2^-24 x terms x |term| / sqrt 2), and chains of a whole stage (~350 sources) put the 99.9 %

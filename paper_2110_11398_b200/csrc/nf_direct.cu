@@ -154,6 +154,13 @@ struct Partial {
 };
 
 constexpr uint32_t kFull = 0xffffffffu;
+// -DNF_DEBUG_BOUNDS: every table index of the sparse path is checked on the device and a violation traps (the launch then
+// fails with an error instead of reading or writing out of bounds); compute-sanitizer is not available on every box
+#ifdef NF_DEBUG_BOUNDS
+#define NF_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define NF_CHECK(cond) do { } while (0)
+#endif
 #ifndef NF_UNROLL_SOFT
 #define NF_UNROLL_SOFT 2
 #endif
@@ -471,6 +478,7 @@ __device__ __forceinline__ void producer(const AccelArgs &a, SharedStorageT<NARR
                                     const uint32_t e0 = row + (uint32_t)(sa[q] + sh[q]), al = e0 & ~3u;      // aligned superset of [e0, e0 + nc]
                                     const uint32_t cnt = (e0 + (uint32_t)nc + 1u - al + 3u) & ~3u;
                                     d.seg[q].ps0 = (int)(psb + (e0 - al));
+                                    NF_CHECK(psb + cnt <= (uint32_t)kPsMax && slot + len[q] <= (uint32_t)kTile && (len[q] & 3u) == 0 && (g0[q] & 3u) == 0);
                                     tma_load_1d(&sm.ps[stage][psb], a.poff + al, cnt * 4u, &sm.full[stage]);
                                     extra_tx += cnt * 4u;
                                     psb += cnt;
@@ -714,8 +722,10 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                     auto cell = [&](const int i, int &slot, int &nsl, double &czs) {
                         const int q = i < n0 ? 0 : (i < n01 ? 1 : 2), li = i - (q == 0 ? 0 : (q == 1 ? n0 : n01));
                         const StageDesc::Seg sg = d.seg[q];
+                        NF_CHECK(i >= 0 && i < np && li >= 0 && li < sg.ncell && sg.ps0 >= 0 && sg.ps0 + li + 1 < kPsMax);
                         const uint32_t p0 = ps[sg.ps0 + li], p1 = ps[sg.ps0 + li + 1];
                         slot = sg.slot0 + (int)(p0 - ps[sg.ps0]); nsl = (int)(p1 - p0);
+                        NF_CHECK(slot >= 0 && nsl >= 0 && slot + nsl <= kTile && (slot & 3) == 0 && (nsl & 3) == 0);
                         czs = ((double)(float)((double)(sg.jw0 + li) * a.k.cell_w) + sg.wz) * a.k.scale;
                     };
                     for (int i = wlo + lane; i <= whi; i += 32) {
@@ -732,7 +742,9 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                     }
                 } else {
                     for (int i = wlo + lane; i <= whi; i += 32) {
+                        NF_CHECK(i >= 0 && i < np && np <= kMaxPieces);
                         const Piece pc = d.pieces[i];
+                        NF_CHECK(pc.sm_off >= 0 && pc.nslots >= 0 && pc.sm_off + pc.nslots <= kTile);
                         for (int q = pc.sm_off >> 2, qe = (pc.sm_off + pc.nslots) >> 2; q < qe; q++) qz[q] = pc.czs;
                     }
                     if (ilo <= ihi) {
@@ -755,6 +767,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
 #pragma unroll 2
                     for (int it = 0; it < cmax; it++) {
                         const int q = it < cnt ? qlo + it : kTile / 4;
+                        NF_CHECK(q >= 0 && q <= kTile / 4);
                         const float dzc = (float)(qz[q] - oczs);
                         const float2 nz = make_float2(dzc - zi.x, dzc - zi.y);
                         quad<PACKED, MODE, MASS, MODE == 2 && NF_DENS_QV>(sbase[q], py0[q], pz0[q], MASS ? pm0[q] : one, nx, ny, nz, coef, f);
@@ -777,6 +790,7 @@ __device__ __forceinline__ void consumer(const AccelArgs &a, SharedStorageT<MASS
                 int n4 = 0, sm_off = 0;
                 double czs = 0.0;
                 if (valid) {
+                    NF_CHECK(np <= kMaxPieces);
                     const Piece pc = d.pieces[idx];
                     n4 = pc.nslots >> 2; sm_off = pc.sm_off; czs = pc.czs;
                 }

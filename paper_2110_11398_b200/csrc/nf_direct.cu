@@ -29,7 +29,11 @@
 //   * the spline is evaluated only where it can matter: a source cell whose nearest face is farther than eps_s
 //     from every sink of the warp takes the pure Newtonian body; the others take min(r^2) over each quad of
 //     sources, vote, and evaluate (C r + B) r + A and the min only when some lane has a pair inside eps_s;
-//   * FP32 FMA chain per (sink, stage), stage partials added in FP64 (two-level accumulation);
+//   * sparse windows (flat units: their cells hold few slots) walk a lane's 2R+1 stencil cells of a column as ONE run of
+//     quads (flat loop); when the whole z-run of a neighbour column fits a stage the producer copies the run's padded
+//     offsets instead of building a per-cell table (lean stage).  nf_bin sorts the flat units behind all the others and
+//     nf_accel runs the two groups as two launches: the stepped units in instances compiled without the flat loop;
+//   * FP32 FMA chain per (sink, source cell), partials added in FP64 in shared memory (two-level accumulation);
 //   * the epilogue writes acc[perm[s]] directly (S7 fused, no sorted acceleration buffer).
 #include "nf_internal.h"
 
